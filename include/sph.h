@@ -1,0 +1,174 @@
+/*
+ * sph.h -- C ABI of the B200-native SPH right-hand-side library (libsph_b200.so).
+ *
+ * The library evaluates, on one NVIDIA B200 (sm_100a), the per-timestep right-hand side of
+ * the solid-body SPH method with Barnes-Hut self-gravity of Schaefer et al.,
+ * arXiv:1604.03290 ("PAPER.md" below = /root/reference/PAPER.md of the build):
+ *
+ *   tree build -> pseudo-particles -> interaction-partner search -> SPH sums -> self-gravity
+ *   (the sub-step list of PAPER.md:693, section 6.2), plus the predictor-corrector step of
+ *   PAPER.md:388-394.
+ *
+ * Conventions
+ *   - All real data are FP64, indices int32, Morton keys uint64.  Arrays are structure-of-arrays,
+ *     one contiguous array per quantity, length n unless stated otherwise.
+ *   - Users see ORIGINAL particle order everywhere.  The Morton-sorted order is internal.
+ *   - `h` is the paper's smoothing length: the kernel vanishes for r/h > 1 (eq. 25).
+ *   - Stress components are stored as S[6] = (xx, xy, xz, yy, yz, zz); in 2-D only xx, xy, yy are used.
+ *   - The damage state variable is dmg = d^(1/3) in [0, 1] (eq. 46).
+ *   - Every pointer argument is documented as HOST or DEVICE.  The library never allocates device
+ *     memory: the caller passes one device workspace of sph_workspace_bytes() bytes and owns it.
+ *   - All calls return an int status (0 = SPH_OK, negative = error); nothing throws or aborts.
+ *     Work is enqueued asynchronously on the stream given to sph_create; calls that return data to
+ *     the HOST (sph_download with dst_is_device = 0, the sph_get_* calls, sph_sync) synchronise that
+ *     stream and also report device-side failures (list overflow, stack overflow) recorded earlier.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns SPH_ERR_CUDA.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sph_ctx sph_ctx; /* opaque; host object created by sph_create */
+
+enum {
+    SPH_OK = 0,
+    SPH_ERR_ARG = -1,                /* bad argument (NULL, n < 1, dim not 2/3, theta >= 1/sqrt(dim), ...) */
+    SPH_ERR_STATE = -2,              /* call order: e.g. sph_rhs before sph_find_neighbours */
+    SPH_ERR_WORKSPACE = -3,          /* workspace too small or misaligned (256 B) */
+    SPH_ERR_NEIGHBOUR_OVERFLOW = -4, /* a particle has more than max_neighbours partners */
+    SPH_ERR_TREE_DEPTH = -5,         /* traversal stack exhausted (too many particles share one key) */
+    SPH_ERR_CUDA = -6                /* CUDA runtime error or no device; see sph_last_error */
+};
+
+enum {
+    SPH_F_SOLID = 1,         /* deviatoric stress S, correction tensor, dS/dt */
+    SPH_F_PLASTIC = 2,       /* von Mises limiter */
+    SPH_F_DAMAGE = 4,        /* Grady-Kipp damage */
+    SPH_F_GRAVITY = 8,       /* Barnes-Hut self-gravity */
+    SPH_F_VARIABLE_H = 16,   /* mean smoothing length per pair + eq. 73 update */
+    SPH_F_DENSITY_SUM = 32   /* rho by kernel sum, eq. 28, instead of continuity */
+};
+
+enum { SPH_EOS_IDEAL_GAS = 0, SPH_EOS_MURNAGHAN = 1, SPH_EOS_TILLOTSON = 2 };
+
+/* Material parameters. Murnaghan: PAPER.md:120 (eq. 13). Tillotson: PAPER.md:128-137 (eqs. 14-15).
+ * mu: shear modulus (eq. 7); Y0: von Mises yield stress (eq. 17), 0 = no limiter for this material;
+ * brittle: 1 = damage model applies to this material. */
+typedef struct {
+    int32_t eos;
+    int32_t brittle;
+    double rho0, K0, nM, gamma;
+    double tA, tB, tE0, tEiv, tEcv, ta, tb, talpha, tbeta;
+    double mu, Y0;
+} sph_material;
+
+typedef struct {
+    int32_t dim;            /* 2 or 3 */
+    int32_t flags;          /* SPH_F_* */
+    int32_t n_materials;
+    int32_t morton_bits;    /* bits per dimension of the Morton key, 1..21; 0 = default 21 */
+    int32_t max_neighbours; /* capacity of one interaction list (PAPER.md:481 interactionsList); 0 = 128 */
+    int32_t n_des;          /* desired partner count of eq. 73 */
+    int32_t h_iters;        /* eq.-73 updates per sph_find_neighbours (only with SPH_F_VARIABLE_H) */
+    int32_t reserved;
+    int64_t n;              /* particles */
+    int64_t n_flaws;        /* total flaw thresholds (length of flaw_eps); 0 without damage */
+    double theta;           /* opening angle of eq. 50; must be < 1/sqrt(dim) */
+    double G;               /* gravitational constant */
+    double eps_soft;        /* Plummer softening length added in eq. 51 */
+    double av_alpha, av_beta, av_eps; /* artificial viscosity, eqs. 32-33 */
+} sph_config;
+
+/* Input state, original order.  NULL members are left unchanged (or zero on first upload).
+ * x[2], v[2] and the z components of S are ignored when dim == 2.
+ * flaw_off has n+1 entries (CSR into flaw_eps, thresholds ascending per particle; eq. 45). */
+typedef struct {
+    const double *x[3], *v[3], *m, *rho, *u, *S[6], *dmg, *h;
+    const int32_t *mat, *n_act;
+    const int64_t *flaw_off;
+    const double *flaw_eps;
+} sph_state_in;
+
+/* Output buffers, original order, each of length n; NULL members are skipped.
+ * State: x, v, rho, u, S, dmg, h, n_act.  Rates of the LAST evaluation: drho (eq. 29), dv (eqs. 30/34,
+ * SPH part only), du (eq. 31), dS (eqs. 7-10), ddmg (eq. 46, rate of dmg = d^(1/3)), ag (eq. 51,
+ * gravitational acceleration), p and cs (equation of state), strain (eq. 48), n_act_new (activated
+ * flaws found by the last evaluation, latched with the committed count), nb_count (partners). */
+typedef struct {
+    double *x[3], *v[3], *rho, *u, *S[6], *dmg, *h;
+    double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *p, *cs, *strain;
+    int32_t *n_act, *n_act_new, *nb_count;
+} sph_state_out;
+
+/* Bytes of device workspace sph_create needs for this configuration (0 on invalid config). */
+size_t sph_workspace_bytes(const sph_config *cfg);
+
+/* cfg, materials: HOST.  d_workspace: DEVICE, 256-byte aligned, >= sph_workspace_bytes(cfg).
+ * cuda_stream: a cudaStream_t (NULL = default stream).  *out receives the context. */
+int sph_create(const sph_config *cfg, const sph_material *materials, void *d_workspace,
+               size_t workspace_bytes, void *cuda_stream, sph_ctx **out);
+void sph_destroy(sph_ctx *ctx);
+
+/* Copy particle state into the context (original order). src_is_device: 1 = DEVICE pointers,
+ * 0 = HOST pointers (pinned memory makes the copy asynchronous). Invalidates tree and lists. */
+int sph_upload(sph_ctx *ctx, const sph_state_in *src, int src_is_device);
+
+/* A1-A4: bounding cube (eq. 67) -> Morton keys -> radix sort + SoA reorder -> octree topology ->
+ * pseudo-particles (mass, centre of mass) with bounding boxes and hmax. */
+int sph_build_tree(sph_ctx *ctx);
+
+/* A5: interaction partners b != a with r_ab < h, or r_ab < (h_a+h_b)/2 with
+ * SPH_F_VARIABLE_H (eq. 72), preceded by h_iters updates of eq. 73. Needs sph_build_tree. */
+int sph_find_neighbours(sph_ctx *ctx);
+
+/* A6-A10: [density sum eq. 28] -> EoS, limiter, damaged stress -> pair sums eqs. 29-34, 41-44 ->
+ * dS/dt (eqs. 7-10) and damage rate (eqs. 46-49). Needs tree and lists. */
+int sph_rhs(sph_ctx *ctx);
+
+/* A11: Barnes-Hut walk, eqs. 50-51, monopoles only. Needs sph_build_tree. Zero without SPH_F_GRAVITY. */
+int sph_gravity(sph_ctx *ctx);
+
+/* One complete right-hand-side evaluation: build_tree, find_neighbours, rhs, gravity. */
+int sph_evaluate(sph_ctx *ctx);
+
+/* A12: predictor-corrector step (eqs. 52-53): two complete evaluations and two updates. */
+int sph_step(sph_ctx *ctx, double dt);
+
+/* Copy state and/or the rates of the last evaluation out, original order.
+ * dst_is_device: 1 = DEVICE buffers (asynchronous), 0 = HOST buffers (synchronises). */
+int sph_download(sph_ctx *ctx, const sph_state_out *dst, int dst_is_device);
+
+/* Wait for all enqueued work; returns the first device-side failure if any. */
+int sph_sync(sph_ctx *ctx);
+
+/* ---- inspection for parity tests (HOST buffers; synchronise) ---- */
+/* keys[n]: sorted Morton keys; perm[n]: perm[i] = original index of the i-th sorted particle.
+ * root[4]: xmin, ymin, zmin of the root cube and its edge s0 (eq. 67). Any pointer may be NULL. */
+int sph_get_order(sph_ctx *ctx, uint64_t *keys, int32_t *perm, double *root);
+/* Number of internal octree nodes. */
+int sph_get_tree_size(sph_ctx *ctx, int32_t *n_nodes);
+/* Node list in the library's depth-first order (sorted by (lo, level)); each array n_nodes long,
+ * com/bmin/bmax 3*n_nodes (node-major). child: (2^dim)*n_nodes entries: >= 0 node index,
+ * -1 empty, -2 leaf; child_lo: (2^dim+1)*n_nodes boundaries into the sorted order. NULL = skip. */
+int sph_get_tree(sph_ctx *ctx, int32_t *level, uint64_t *prefix, int32_t *lo, int32_t *hi,
+                 double *mass, double *com, double *bmin, double *bmax, double *hmax,
+                 int32_t *child, int32_t *child_lo);
+/* CSR partner lists in ORIGINAL indices, ascending per particle. off[n+1]; idx[cap]. Returns
+ * SPH_ERR_ARG if cap is too small (off is still filled, so off[n] tells the needed size). */
+int sph_get_neighbours(sph_ctx *ctx, int64_t *off, int32_t *idx, int64_t cap);
+/* Per-call kernel time accounting: number of kernels launched by this context so far. */
+int64_t sph_launch_count(sph_ctx *ctx);
+
+const char *sph_last_error(sph_ctx *ctx);
+const char *sph_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

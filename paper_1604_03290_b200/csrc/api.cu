@@ -1,0 +1,529 @@
+// C ABI of libsph_b200.so (declared in include/sph.h): context, workspace layout, upload/download,
+// call-order checks, the predictor-corrector update (A12) and the inspection calls used by the
+// parity tests.  Every compute step runs in the kernels of order.cu / tree.cu / neigh.cu / rhs.cu /
+// gravity.cu; this file holds host logic and three small per-particle kernels (update, unsort).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sph_internal.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// workspace layout: one bump allocation pass, used both to size and to carve
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct Bump {
+    char *base;
+    size_t off;
+    template <class T> T *take(size_t count) {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? (T *)(base + off) : (T *)nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+int cfg_cap(const sph_config *c) { return c->max_neighbours > 0 ? c->max_neighbours : 128; }
+int cfg_L(const sph_config *c) { return c->morton_bits > 0 ? c->morton_bits : 21; }
+
+bool cfg_ok(const sph_config *c) {
+    if (!c) return false;
+    if (c->dim != 2 && c->dim != 3) return false;
+    if (c->n < 1 || c->n > (int64_t)0x3fffffff) return false;
+    if (c->n_materials < 1 || c->n_materials > SPH_MAX_MAT) return false;
+    if (c->morton_bits < 0 || c->morton_bits > 21) return false;
+    if (c->max_neighbours < 0 || c->max_neighbours > 4096) return false;
+    if (c->n_flaws < 0) return false;
+    if ((c->flags & SPH_F_GRAVITY) && !(c->theta >= 0.0 && c->theta * c->theta * c->dim < 1.0)) return false;
+    if ((c->flags & SPH_F_VARIABLE_H) && c->h_iters > 0 && c->n_des < 1) return false;
+    return true;
+}
+
+// Fills d with pointers into base (or only measures when base == nullptr). Returns bytes used.
+size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
+    Bump b{base, 0};
+    const size_t n = (size_t)c->n;
+    const int D = c->dim, NC = 1 << D;
+    const size_t groups = (n + 31) / 32;
+    Dev z;
+    memset(&z, 0, sizeof(z));
+    // master state: x3 v3 rho u S6 dmg contiguous (the RK2 base copy mirrors these 15 arrays)
+    double *st = b.take<double>(15 * n);
+    for (int a = 0; a < 3; ++a) { z.x[a] = st ? st + (size_t)a * n : nullptr; z.v[a] = st ? st + (size_t)(3 + a) * n : nullptr; }
+    z.rho = st ? st + 6 * n : nullptr;
+    z.u = st ? st + 7 * n : nullptr;
+    for (int k = 0; k < 6; ++k) z.S[k] = st ? st + (size_t)(8 + k) * n : nullptr;
+    z.dmg = st ? st + 14 * n : nullptr;
+    z.m = b.take<double>(n);
+    z.h = b.take<double>(n);
+    z.mat = b.take<int>(n);
+    z.n_act = b.take<int>(n);
+    z.flaw_off = b.take<i64>(n + 1);
+    z.flaw_eps = b.take<double>((size_t)std::max<int64_t>(c->n_flaws, 1));
+    z.q0 = b.take<double>(15 * n);
+    for (int a = 0; a < 3; ++a) { z.sx[a] = b.take<double>(n); z.sv[a] = b.take<double>(n); }
+    z.sm = b.take<double>(n); z.srho = b.take<double>(n); z.su = b.take<double>(n);
+    for (int k = 0; k < 6; ++k) z.sS[k] = b.take<double>(n);
+    z.sdmg = b.take<double>(n); z.sh = b.take<double>(n);
+    z.smat = b.take<int>(n);
+    for (int k = 0; k < 2; ++k) { z.key[k] = b.take<u64>(n); z.idx[k] = b.take<int>(n); }
+    z.hist = b.take<unsigned>(256 * ((n + 4095) / 4096) + 256);
+    z.partial = b.take<double>(1024 * 6);
+    z.root = b.take<DevRoot>(1);
+    z.status = b.take<DevStatus>(1);
+    for (int k = 0; k < 2; ++k) { z.nkey[k] = b.take<u64>(n); z.nhi[k] = b.take<int>(n); }
+    z.nlevel = b.take<int>(n); z.nlo = b.take<int>(n); z.nhi_s = b.take<int>(n); z.nskip = b.take<int>(n);
+    z.child = b.take<int>(n * NC);
+    z.child_lo = b.take<int>(n * (NC + 1));
+    z.nmass = b.take<double>(n);
+    for (int a = 0; a < 3; ++a) { z.ncom[a] = b.take<double>(n); z.nbmin[a] = b.take<double>(n); z.nbmax[a] = b.take<double>(n); }
+    z.nhmax = b.take<double>(n); z.ns2 = b.take<double>(n);
+    z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);
+    z.nb_cnt = b.take<int>(n); z.own_cnt = b.take<int>(n);
+    z.p = b.take<double>(n); z.cs = b.take<double>(n); z.vol = b.take<double>(n);
+    for (int k = 0; k < 6; ++k) z.sr2[k] = b.take<double>(n);
+    z.drho = b.take<double>(n); z.du = b.take<double>(n); z.ddmg = b.take<double>(n); z.strain = b.take<double>(n);
+    for (int a = 0; a < 3; ++a) { z.dv[a] = b.take<double>(n); z.ag[a] = b.take<double>(n); }
+    for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(n);
+    z.n_act_new = b.take<int>(n);
+    z.stage = b.take<double>(n);
+    z.stage_i = b.take<int>(n);
+    Mats *md = b.take<Mats>(1);
+    if (mats_dev) *mats_dev = md;
+    if (d) *d = z;
+    return (b.off + 255) & ~(size_t)255;
+}
+
+int fail(sph_ctx *ctx, int code, const char *msg) {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", msg);
+    return code;
+}
+
+int check_cuda(sph_ctx *ctx, const char *where) {
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) return SPH_OK;
+    snprintf(ctx->err, sizeof(ctx->err), "%s: %s", where, cudaGetErrorString(e));
+    return SPH_ERR_CUDA;
+}
+
+}  // namespace
+
+struct sph_ctx_ext {
+    sph_ctx c;
+    Mats *mats_dev;
+};
+
+static inline sph_ctx_ext *ext(sph_ctx *c) { return (sph_ctx_ext *)c; }
+const sph_material *sph_dev_mats(sph_ctx *ctx) { return ext(ctx)->mats_dev->m; }
+
+// ------------------------------------------------------------------------------------------------
+// small per-particle kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_unsort_d(const double *__restrict__ src, const int *__restrict__ perm, double *__restrict__ dst, int n) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[perm[i]] = src[i];
+}
+__global__ void k_unsort_i(const int *__restrict__ src, const int *__restrict__ perm, int *__restrict__ dst, int n) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[perm[i]] = src[i];
+}
+__global__ void k_fill_d(double *dst, double v, size_t n) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = v;
+}
+
+// A12, PAPER.md:388-394 (eqs. 52-53): q <- q0 + c * f, f = rates of the last evaluation (sorted
+// order, scattered through perm), dx/dt = v of the evaluated state (eq. 39 without XSPH).
+// Every product and sum is rounded separately (reading O6).  After the update: dmg clamped to
+// [0, (n_act/n_tot)^(1/3)] (eq. 47), S <- f_Y S (eq. 16); n_act committed only when commit != 0.
+__global__ void k_update(Dev d, const sph_material *mats, double c, int commit) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const size_t n = (size_t)d.n;
+    const int o = d.perm[i];
+    const double *q0 = d.q0;
+    const int D = d.D;
+    for (int a = 0; a < 3; ++a) {
+        if (a < D) {
+            const double vel = d.v[a][o];
+            d.x[a][o] = __dadd_rn(q0[(size_t)a * n + o], __dmul_rn(c, vel));
+            d.v[a][o] = __dadd_rn(q0[(size_t)(3 + a) * n + o], __dmul_rn(c, __dadd_rn(d.dv[a][i], d.ag[a][i])));
+        } else {
+            d.x[a][o] = 0.0;
+            d.v[a][o] = 0.0;
+        }
+    }
+    if (!(d.flags & SPH_F_DENSITY_SUM)) d.rho[o] = __dadd_rn(q0[6 * n + o], __dmul_rn(c, d.drho[i]));
+    d.u[o] = __dadd_rn(q0[7 * n + o], __dmul_rn(c, d.du[i]));
+    const sph_material &mt = mats[d.smat[i]];
+    if (d.flags & SPH_F_SOLID) {
+        double S[6];
+        for (int k = 0; k < 6; ++k) S[k] = __dadd_rn(q0[(size_t)(8 + k) * n + o], __dmul_rn(c, d.dS[k][i]));
+        if ((d.flags & SPH_F_PLASTIC) && mt.Y0 > 0.0) {
+            double SS;
+            if (D == 3) {
+                const double dg = __dadd_rn(__dadd_rn(__dmul_rn(S[0], S[0]), __dmul_rn(S[3], S[3])), __dmul_rn(S[5], S[5]));
+                const double of = __dadd_rn(__dadd_rn(__dmul_rn(S[1], S[1]), __dmul_rn(S[2], S[2])), __dmul_rn(S[4], S[4]));
+                SS = __dadd_rn(dg, __dmul_rn(2.0, of));
+            } else {
+                SS = __dadd_rn(__dadd_rn(__dmul_rn(S[0], S[0]), __dmul_rn(S[3], S[3])), __dmul_rn(2.0, __dmul_rn(S[1], S[1])));
+            }
+            const double J2 = __dmul_rn(0.5, SS), Y2 = __dmul_rn(mt.Y0, mt.Y0), J3 = __dmul_rn(3.0, J2);
+            if (J3 > Y2) {
+                const double fY = __ddiv_rn(Y2, J3);
+                for (int k = 0; k < 6; ++k) S[k] = __dmul_rn(S[k], fY);
+            }
+        }
+        for (int k = 0; k < 6; ++k) d.S[k][o] = S[k];
+    }
+    if (d.flags & SPH_F_DAMAGE) {
+        const i64 ntot = d.flaw_off[o + 1] - d.flaw_off[o];
+        const int nact = d.n_act_new[i];
+        const double dmax = (ntot > 0) ? cbrt((double)nact / (double)ntot) : 0.0;
+        double g = __dadd_rn(q0[14 * n + o], __dmul_rn(c, d.ddmg[i]));
+        g = fmin(fmax(g, 0.0), dmax);
+        d.dmg[o] = g;
+        if (commit) d.n_act[o] = nact;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+size_t sph_workspace_bytes(const sph_config *cfg) {
+    if (!cfg_ok(cfg)) return 0;
+    return carve(cfg, nullptr, nullptr, nullptr);
+}
+
+int sph_create(const sph_config *cfg, const sph_material *materials, void *d_workspace, size_t workspace_bytes,
+               void *cuda_stream, sph_ctx **out) {
+    if (!out) return SPH_ERR_ARG;
+    *out = nullptr;
+    if (!cfg_ok(cfg) || !materials) return SPH_ERR_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return SPH_ERR_CUDA; }
+    if (!d_workspace || ((uintptr_t)d_workspace & 255)) return SPH_ERR_WORKSPACE;
+    if (workspace_bytes < carve(cfg, nullptr, nullptr, nullptr)) return SPH_ERR_WORKSPACE;
+    sph_ctx_ext *e = new (std::nothrow) sph_ctx_ext();
+    if (!e) return SPH_ERR_ARG;
+    memset(e, 0, sizeof(*e));
+    sph_ctx *c = &e->c;
+    c->cfg = *cfg;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws = d_workspace;
+    c->ws_bytes = workspace_bytes;
+    carve(cfg, (char *)d_workspace, &c->d, &e->mats_dev);
+    Dev &d = c->d;
+    d.D = cfg->dim; d.L = cfg_L(cfg); d.flags = cfg->flags; d.cap = cfg_cap(cfg);
+    d.n = (int)cfg->n; d.n_des = cfg->n_des;
+    d.theta2 = cfg->theta * cfg->theta;
+    d.G = cfg->G;
+    d.eps2 = cfg->eps_soft * cfg->eps_soft;
+    d.av_alpha = cfg->av_alpha; d.av_beta = cfg->av_beta; d.av_eps = cfg->av_eps;
+    memset(&c->mats, 0, sizeof(c->mats));
+    for (int k = 0; k < cfg->n_materials; ++k) c->mats.m[k] = materials[k];
+    cudaMemcpyAsync(e->mats_dev, &c->mats, sizeof(Mats), cudaMemcpyHostToDevice, c->stream);
+    cudaMemsetAsync(d.status, 0, sizeof(DevStatus), c->stream);
+    // defaults for state members never uploaded
+    const size_t n = (size_t)d.n;
+    cudaMemsetAsync(d.x[0], 0, 15 * n * sizeof(double), c->stream);
+    cudaMemsetAsync(d.m, 0, n * sizeof(double), c->stream);
+    cudaMemsetAsync(d.h, 0, n * sizeof(double), c->stream);
+    cudaMemsetAsync(d.mat, 0, n * sizeof(int), c->stream);
+    cudaMemsetAsync(d.n_act, 0, n * sizeof(int), c->stream);
+    cudaMemsetAsync(d.flaw_off, 0, (n + 1) * sizeof(i64), c->stream);
+    cudaStreamSynchronize(c->stream);   // c->mats is pageable host memory: finish the copy now
+    int rc = check_cuda(c, "sph_create");
+    if (rc != SPH_OK) { delete e; return rc; }
+    *out = c;
+    return SPH_OK;
+}
+
+void sph_destroy(sph_ctx *ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    delete ext(ctx);
+}
+
+int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
+    if (!ctx || !s) return SPH_ERR_ARG;
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    auto cp = [&](void *dst, const void *src, size_t bytes) {
+        if (src && bytes) cudaMemcpyAsync(dst, src, bytes, kind, ctx->stream);
+    };
+    for (int a = 0; a < d.D; ++a) { cp(d.x[a], s->x[a], n * 8); cp(d.v[a], s->v[a], n * 8); }
+    cp(d.m, s->m, n * 8); cp(d.rho, s->rho, n * 8); cp(d.u, s->u, n * 8); cp(d.dmg, s->dmg, n * 8); cp(d.h, s->h, n * 8);
+    for (int k = 0; k < 6; ++k) cp(d.S[k], s->S[k], n * 8);
+    cp(d.mat, s->mat, n * 4); cp(d.n_act, s->n_act, n * 4);
+    cp(d.flaw_off, s->flaw_off, (n + 1) * 8);
+    cp(d.flaw_eps, s->flaw_eps, (size_t)ctx->cfg.n_flaws * 8);
+    if (!src_is_device) cudaStreamSynchronize(ctx->stream);   // caller may free or reuse its buffers
+    ctx->have_state = 1; ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
+    return check_cuda(ctx, "sph_upload");
+}
+
+int sph_build_tree(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_build_tree before sph_upload");
+    sph_stage_order(ctx);
+    sph_stage_tree(ctx);
+    ctx->have_tree = 1; ctx->have_lists = 0; ctx->have_rates = 0;
+    return check_cuda(ctx, "sph_build_tree");
+}
+
+int sph_find_neighbours(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_tree) return fail(ctx, SPH_ERR_STATE, "sph_find_neighbours before sph_build_tree");
+    sph_stage_neigh(ctx);
+    ctx->have_lists = 1;
+    return check_cuda(ctx, "sph_find_neighbours");
+}
+
+int sph_rhs(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_tree || !ctx->have_lists) return fail(ctx, SPH_ERR_STATE, "sph_rhs before sph_find_neighbours");
+    sph_stage_rhs(ctx);
+    ctx->have_rates |= 1;
+    return check_cuda(ctx, "sph_rhs");
+}
+
+int sph_gravity(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_tree) return fail(ctx, SPH_ERR_STATE, "sph_gravity before sph_build_tree");
+    sph_stage_gravity(ctx);
+    ctx->have_rates |= 2;
+    return check_cuda(ctx, "sph_gravity");
+}
+
+int sph_evaluate(sph_ctx *ctx) {
+    int rc;
+    if ((rc = sph_build_tree(ctx)) != SPH_OK) return rc;
+    if ((rc = sph_find_neighbours(ctx)) != SPH_OK) return rc;
+    if ((rc = sph_rhs(ctx)) != SPH_OK) return rc;
+    return sph_gravity(ctx);
+}
+
+int sph_step(sph_ctx *ctx, double dt) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    int rc;
+    cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
+    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), 0.5 * dt, 0);   // eq. 52
+    ctx->launches += 1;
+    if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
+    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, 1);         // eq. 53
+    ctx->launches += 1;
+    ctx->have_tree = ctx->have_lists = 0;   // the state moved on; the rates stay readable
+    return check_cuda(ctx, "sph_step");
+}
+
+static int device_flags(sph_ctx *ctx) {
+    DevStatus st;
+    if (cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream) != cudaSuccess ||
+        cudaStreamSynchronize(ctx->stream) != cudaSuccess)
+        return check_cuda(ctx, "status") == SPH_OK ? SPH_ERR_CUDA : SPH_ERR_CUDA;
+    if (st.err_nb_overflow) {
+        snprintf(ctx->err, sizeof(ctx->err), "interaction list overflow: %d partners > max_neighbours %d", st.nb_max, ctx->d.cap);
+        return SPH_ERR_NEIGHBOUR_OVERFLOW;
+    }
+    if (st.err_stack) return fail(ctx, SPH_ERR_TREE_DEPTH, "traversal stack exhausted");
+    return check_cuda(ctx, "sync");
+}
+
+int sph_sync(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
+    return device_flags(ctx);
+}
+
+int sph_download(sph_ctx *ctx, const sph_state_out *o, int dst_is_device) {
+    if (!ctx || !o) return SPH_ERR_ARG;
+    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_download before sph_upload");
+    Dev &d = ctx->d;
+    const int n = d.n;
+    const size_t nb = (size_t)n * 8;
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    auto plain = [&](void *dst, const void *src, size_t bytes) {
+        if (dst) cudaMemcpyAsync(dst, src, bytes, kind, ctx->stream);
+    };
+    for (int a = 0; a < 3; ++a) { plain(o->x[a], d.x[a], nb); plain(o->v[a], d.v[a], nb); }
+    plain(o->rho, d.rho, nb); plain(o->u, d.u, nb); plain(o->dmg, d.dmg, nb); plain(o->h, d.h, nb);
+    for (int k = 0; k < 6; ++k) plain(o->S[k], d.S[k], nb);
+    plain(o->n_act, d.n_act, (size_t)n * 4);
+    const bool want_rates = o->drho || o->dv[0] || o->dv[1] || o->dv[2] || o->du || o->ddmg || o->ag[0] || o->ag[1] ||
+                            o->ag[2] || o->p || o->cs || o->strain || o->n_act_new || o->nb_count || o->dS[0] ||
+                            o->dS[1] || o->dS[2] || o->dS[3] || o->dS[4] || o->dS[5];
+    if (want_rates && !ctx->have_rates) return fail(ctx, SPH_ERR_STATE, "sph_download of rates before an evaluation");
+    const int gb = sph_ceil_div(n, 256);
+    auto unsort_d = [&](double *dst, const double *src, bool present) {
+        if (!dst) return;
+        if (!present) {   // quantity not computed under the current flags: zeros
+            if (dst_is_device) { k_fill_d<<<gb, 256, 0, ctx->stream>>>(dst, 0.0, (size_t)n); ctx->launches += 1; }
+            else memset(dst, 0, nb);
+            return;
+        }
+        if (dst_is_device) {
+            k_unsort_d<<<gb, 256, 0, ctx->stream>>>(src, d.perm, dst, n);
+        } else {
+            k_unsort_d<<<gb, 256, 0, ctx->stream>>>(src, d.perm, d.stage, n);
+            cudaMemcpyAsync(dst, d.stage, nb, cudaMemcpyDeviceToHost, ctx->stream);
+            cudaStreamSynchronize(ctx->stream);   // stage is reused by the next member
+        }
+        ctx->launches += 1;
+    };
+    auto unsort_i = [&](int *dst, const int *src, bool present) {
+        if (!dst) return;
+        if (!present) {
+            if (dst_is_device) cudaMemsetAsync(dst, 0, (size_t)n * 4, ctx->stream);
+            else memset(dst, 0, (size_t)n * 4);
+            return;
+        }
+        if (dst_is_device) {
+            k_unsort_i<<<gb, 256, 0, ctx->stream>>>(src, d.perm, dst, n);
+        } else {
+            k_unsort_i<<<gb, 256, 0, ctx->stream>>>(src, d.perm, d.stage_i, n);
+            cudaMemcpyAsync(dst, d.stage_i, (size_t)n * 4, cudaMemcpyDeviceToHost, ctx->stream);
+            cudaStreamSynchronize(ctx->stream);
+        }
+        ctx->launches += 1;
+    };
+    const bool sph = (ctx->have_rates & 1) != 0, grav = (ctx->have_rates & 2) != 0;
+    const bool solid = sph && (d.flags & SPH_F_SOLID), dam = sph && (d.flags & SPH_F_DAMAGE);
+    unsort_d(o->drho, d.drho, sph); unsort_d(o->du, d.du, sph);
+    for (int a = 0; a < 3; ++a) { unsort_d(o->dv[a], d.dv[a], sph); unsort_d(o->ag[a], d.ag[a], grav); }
+    for (int k = 0; k < 6; ++k) unsort_d(o->dS[k], d.dS[k], solid);
+    unsort_d(o->ddmg, d.ddmg, dam); unsort_d(o->strain, d.strain, dam);
+    unsort_d(o->p, d.p, sph); unsort_d(o->cs, d.cs, sph);
+    unsort_i(o->n_act_new, d.n_act_new, dam);
+    unsort_i(o->nb_count, d.nb_cnt, ctx->have_lists || sph);
+    if (!dst_is_device) return device_flags(ctx);
+    return check_cuda(ctx, "sph_download");
+}
+
+int64_t sph_launch_count(sph_ctx *ctx) { return ctx ? ctx->launches : 0; }
+const char *sph_last_error(sph_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+const char *sph_version(void) { return "sph-b200 0.1 (sm_100a, FP64)"; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// inspection for the parity tests (HOST buffers; synchronise)
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+int sph_get_order(sph_ctx *ctx, uint64_t *keys, int32_t *perm, double *root) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_tree) return fail(ctx, SPH_ERR_STATE, "sph_get_order before sph_build_tree");
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    if (keys) cudaMemcpyAsync(keys, d.keys, n * 8, cudaMemcpyDeviceToHost, ctx->stream);
+    if (perm) cudaMemcpyAsync(perm, d.perm, n * 4, cudaMemcpyDeviceToHost, ctx->stream);
+    DevRoot r;
+    cudaMemcpyAsync(&r, d.root, sizeof(r), cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    if (root) { root[0] = r.xmin[0]; root[1] = r.xmin[1]; root[2] = r.xmin[2]; root[3] = r.s0; }
+    return check_cuda(ctx, "sph_get_order");
+}
+
+int sph_get_tree_size(sph_ctx *ctx, int32_t *n_nodes) {
+    if (!ctx || !n_nodes) return SPH_ERR_ARG;
+    if (!ctx->have_tree) return fail(ctx, SPH_ERR_STATE, "sph_get_tree_size before sph_build_tree");
+    DevStatus st;
+    cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    *n_nodes = st.n_nodes;
+    return check_cuda(ctx, "sph_get_tree_size");
+}
+
+int sph_get_tree(sph_ctx *ctx, int32_t *level, uint64_t *prefix, int32_t *lo, int32_t *hi, double *mass, double *com,
+                 double *bmin, double *bmax, double *hmax, int32_t *child, int32_t *child_lo) {
+    int32_t nn = 0;
+    int rc = sph_get_tree_size(ctx, &nn);
+    if (rc != SPH_OK) return rc;
+    Dev &d = ctx->d;
+    const int D = d.D, NC = 1 << D;
+    const size_t m = (size_t)nn;
+    if (m == 0) return SPH_OK;
+    auto get = [&](void *dst, const void *src, size_t bytes) {
+        if (dst) cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    };
+    std::vector<int32_t> lv(m), l0(m);
+    get(lv.data(), d.nlevel, m * 4);
+    get(l0.data(), d.nlo, m * 4);
+    get(hi, d.nhi_s, m * 4);
+    get(mass, d.nmass, m * 8);
+    get(hmax, d.nhmax, m * 8);
+    get(child, d.child, m * NC * 4);
+    get(child_lo, d.child_lo, m * (NC + 1) * 4);
+    std::vector<double> t3[3][3];
+    for (int a = 0; a < 3; ++a) {
+        if (com) { t3[0][a].resize(m); get(t3[0][a].data(), d.ncom[a], m * 8); }
+        if (bmin) { t3[1][a].resize(m); get(t3[1][a].data(), d.nbmin[a], m * 8); }
+        if (bmax) { t3[2][a].resize(m); get(t3[2][a].data(), d.nbmax[a], m * 8); }
+    }
+    std::vector<u64> keys;
+    if (prefix) { keys.resize((size_t)d.n); get(keys.data(), d.keys, (size_t)d.n * 8); }
+    cudaStreamSynchronize(ctx->stream);
+    for (size_t k = 0; k < m; ++k) {
+        if (level) level[k] = lv[k];
+        if (lo) lo[k] = l0[k];
+        if (prefix) prefix[k] = (lv[k] == 0) ? 0ull : (keys[(size_t)l0[k]] >> (D * (d.L - lv[k])));
+        for (int a = 0; a < 3; ++a) {
+            if (com) com[3 * k + a] = t3[0][a][k];
+            if (bmin) bmin[3 * k + a] = t3[1][a][k];
+            if (bmax) bmax[3 * k + a] = t3[2][a][k];
+        }
+    }
+    return check_cuda(ctx, "sph_get_tree");
+}
+
+int sph_get_neighbours(sph_ctx *ctx, int64_t *off, int32_t *idx, int64_t cap) {
+    if (!ctx || !off) return SPH_ERR_ARG;
+    if (!ctx->have_lists) return fail(ctx, SPH_ERR_STATE, "sph_get_neighbours before sph_find_neighbours");
+    int rc = device_flags(ctx);
+    if (rc != SPH_OK) return rc;
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    std::vector<int> cnt(n), perm(n);
+    cudaMemcpyAsync(cnt.data(), d.nb_cnt, n * 4, cudaMemcpyDeviceToHost, ctx->stream);
+    cudaMemcpyAsync(perm.data(), d.perm, n * 4, cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    off[0] = 0;
+    {
+        std::vector<int> co(n);
+        for (size_t i = 0; i < n; ++i) co[(size_t)perm[i]] = cnt[i];
+        for (size_t o = 0; o < n; ++o) off[o + 1] = off[o] + co[o];
+    }
+    if (!idx) return SPH_OK;
+    if (cap < off[n]) return fail(ctx, SPH_ERR_ARG, "sph_get_neighbours: idx too small");
+    // lists are group-transposed on the device: fetch a block of groups at a time
+    const size_t groups = (n + 31) / 32, gcap = (size_t)d.cap * 32;
+    const size_t chunk = std::max<size_t>(1, (64u << 20) / (gcap * 4));
+    std::vector<int> buf(chunk * gcap);
+    for (size_t g0 = 0; g0 < groups; g0 += chunk) {
+        const size_t g1 = std::min(groups, g0 + chunk);
+        cudaMemcpyAsync(buf.data(), d.nb + g0 * gcap, (g1 - g0) * gcap * 4, cudaMemcpyDeviceToHost, ctx->stream);
+        cudaStreamSynchronize(ctx->stream);
+        for (size_t g = g0; g < g1; ++g)
+            for (int lane = 0; lane < 32; ++lane) {
+                const size_t i = g * 32 + lane;
+                if (i >= n) break;
+                int32_t *dst = idx + off[(size_t)perm[i]];
+                const int *src = buf.data() + (g - g0) * gcap + lane;
+                for (int k = 0; k < cnt[i]; ++k) dst[k] = perm[(size_t)src[(size_t)k * 32]];
+                std::sort(dst, dst + cnt[i]);
+            }
+    }
+    return check_cuda(ctx, "sph_get_neighbours");
+}
+
+}  // extern "C"

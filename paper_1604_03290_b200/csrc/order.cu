@@ -1,0 +1,236 @@
+// A1 + A2: root cube, Morton keys, LSD radix sort, SoA reorder.
+//   root cube:  PAPER.md:463-465 (eq. 67); min-corner anchored (reading U12)
+//   keys:       L bits per dimension, x lowest bit of each group (U13); ties by original index
+//   sort:       hand-written 8-bit LSD radix sort (histogram -> scan -> stable scatter)
+//   reorder:    every state array gathered into Morton order so that the tree walks, the partner
+//               search and the pair sums read neighbouring particles from neighbouring addresses.
+#include "sph_internal.cuh"
+
+#define SORT_THREADS 256
+#define SORT_ITEMS 16
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+#define SORT_WARPS (SORT_THREADS / 32)
+
+// ------------------------------------------------------------------------------------------
+// bounding box: per-block partial min/max, then one block finishes and derives s0 and scale
+// ------------------------------------------------------------------------------------------
+__global__ void k_bbox_partial(Dev d, int nblocks) {
+    __shared__ double smin[3][8], smax[3][8];
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n; i += gridDim.x * blockDim.x)
+        for (int a = 0; a < d.D; ++a) {
+            double v = d.x[a][i];
+            lo[a] = fmin(lo[a], v); hi[a] = fmax(hi[a], v);
+        }
+    for (int a = 0; a < 3; ++a)
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) for (int a = 0; a < 3; ++a) { smin[a][w] = lo[a]; smax[a][w] = hi[a]; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int a = 0; a < 3; ++a) {
+            double mn = smin[a][0], mx = smax[a][0];
+            for (int k = 1; k < (int)(blockDim.x >> 5); ++k) { mn = fmin(mn, smin[a][k]); mx = fmax(mx, smax[a][k]); }
+            d.partial[(blockIdx.x * 3 + a) * 2 + 0] = mn;
+            d.partial[(blockIdx.x * 3 + a) * 2 + 1] = mx;
+        }
+    }
+}
+
+__global__ void k_bbox_final(Dev d, int nblocks) {
+    // one warp
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int b = threadIdx.x; b < nblocks; b += 32)
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fmin(lo[a], d.partial[(b * 3 + a) * 2 + 0]);
+            hi[a] = fmax(hi[a], d.partial[(b * 3 + a) * 2 + 1]);
+        }
+    for (int a = 0; a < 3; ++a)
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+    if (threadIdx.x == 0) {
+        double s0 = 0.0;
+        for (int a = 0; a < d.D; ++a) s0 = fmax(s0, __dsub_rn(hi[a], lo[a]));   // eq. 67
+        if (!(s0 > 0.0)) s0 = 1.0;
+        for (int a = 0; a < 3; ++a) d.root->xmin[a] = (a < d.D) ? lo[a] : 0.0;
+        d.root->s0 = s0;
+        d.root->scale = __ddiv_rn(ldexp(1.0, d.L), s0);
+    }
+}
+
+__device__ __forceinline__ u64 spread3(u64 v) {   // 21 bits -> every third bit
+    v &= 0x1fffffull;
+    v = (v | (v << 32)) & 0x1f00000000ffffull;
+    v = (v | (v << 16)) & 0x1f0000ff0000ffull;
+    v = (v | (v << 8)) & 0x100f00f00f00f00full;
+    v = (v | (v << 4)) & 0x10c30c30c30c30c3ull;
+    v = (v | (v << 2)) & 0x1249249249249249ull;
+    return v;
+}
+__device__ __forceinline__ u64 spread2(u64 v) {   // 21 bits -> every second bit
+    v &= 0x1fffffull;
+    v = (v | (v << 16)) & 0x0000ffff0000ffffull;
+    v = (v | (v << 8)) & 0x00ff00ff00ff00ffull;
+    v = (v | (v << 4)) & 0x0f0f0f0f0f0f0f0full;
+    v = (v | (v << 2)) & 0x3333333333333333ull;
+    v = (v | (v << 1)) & 0x5555555555555555ull;
+    return v;
+}
+
+__global__ void k_keys(Dev d) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const double scale = d.root->scale;
+    const u64 gmax = (1ull << d.L) - 1ull;
+    u64 g[3] = {0, 0, 0};
+    for (int a = 0; a < d.D; ++a) {
+        double t = __dmul_rn(__dsub_rn(d.x[a][i], d.root->xmin[a]), scale);
+        u64 gi = (u64)t;                       // truncation; t >= 0
+        g[a] = gi < gmax ? gi : gmax;
+    }
+    u64 key = (d.D == 3) ? (spread3(g[0]) | (spread3(g[1]) << 1) | (spread3(g[2]) << 2))
+                         : (spread2(g[0]) | (spread2(g[1]) << 1));
+    d.key[0][i] = key;
+    d.idx[0][i] = i;
+}
+
+// ------------------------------------------------------------------------------------------
+// radix sort
+// ------------------------------------------------------------------------------------------
+__global__ void k_sort_hist(const u64 *__restrict__ kin, int n_host, const int *n_dev, int shift,
+                            unsigned *hist, int nblocks) {
+    __shared__ unsigned h[256];
+    const int n = n_dev ? *n_dev : n_host;
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    i64 base = (i64)blockIdx.x * SORT_TILE;
+    for (int j = 0; j < SORT_ITEMS; ++j) {
+        i64 i = base + j * SORT_THREADS + threadIdx.x;
+        if (i < n) atomicAdd(&h[(unsigned)(kin[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+}
+
+__global__ void k_sort_scan(unsigned *hist, int total) {   // one block of 1024 threads, exclusive scan
+    __shared__ unsigned part[1024];
+    int per = (total + 1023) / 1024;
+    int b = threadIdx.x * per, e = min(b + per, total);
+    unsigned s = 0;
+    for (int i = b; i < e; ++i) s += hist[i];
+    part[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        unsigned v = (threadIdx.x >= o) ? part[threadIdx.x - o] : 0;
+        __syncthreads();
+        part[threadIdx.x] += v;
+        __syncthreads();
+    }
+    unsigned run = part[threadIdx.x] - s;
+    for (int i = b; i < e; ++i) { unsigned v = hist[i]; hist[i] = run; run += v; }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__restrict__ kout,
+               int *__restrict__ vout, int n_host, const int *n_dev, int shift,
+               const unsigned *__restrict__ offs, int nblocks) {
+    __shared__ unsigned wc[SORT_WARPS][256];
+    __shared__ unsigned gbase[256];
+    const int n = n_dev ? *n_dev : n_host;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int k = threadIdx.x; k < SORT_WARPS * 256; k += SORT_THREADS) (&wc[0][0])[k] = 0;
+    gbase[threadIdx.x] = offs[threadIdx.x * nblocks + blockIdx.x];
+    __syncthreads();
+    const i64 base = (i64)blockIdx.x * SORT_TILE + (i64)w * (32 * SORT_ITEMS);
+    u64 key[SORT_ITEMS];
+    int val[SORT_ITEMS];
+    unsigned rank[SORT_ITEMS];
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int j = 0; j < SORT_ITEMS; ++j) {
+        i64 i = base + j * 32 + lane;
+        bool valid = i < n;
+        key[j] = valid ? kin[i] : 0ull;
+        val[j] = valid ? vin[i] : 0;
+        unsigned dg = (unsigned)(key[j] >> shift) & 255u;
+        unsigned m = __match_any_sync(0xffffffffu, valid ? dg : 256u);
+        unsigned prev = valid ? wc[w][dg] : 0u;
+        __syncwarp();
+        if (valid && (m & lt) == 0) wc[w][dg] = prev + __popc(m);
+        __syncwarp();
+        rank[j] = prev + __popc(m & lt);
+    }
+    __syncthreads();
+    {   // exclusive scan over warps, one digit per thread
+        unsigned run = 0;
+        for (int k = 0; k < SORT_WARPS; ++k) { unsigned t = wc[k][threadIdx.x]; wc[k][threadIdx.x] = run; run += t; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < SORT_ITEMS; ++j) {
+        i64 i = base + j * 32 + lane;
+        if (i < n) {
+            unsigned dg = (unsigned)(key[j] >> shift) & 255u;
+            unsigned pos = gbase[dg] + wc[w][dg] + rank[j];
+            kout[pos] = key[j];
+            vout[pos] = val[j];
+        }
+    }
+}
+
+void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur) {
+    const int nblocks = sph_ceil_div(n_host, SORT_TILE);
+    int c = *cur;
+    for (int shift = 0; shift < bits; shift += 8) {
+        k_sort_hist<<<nblocks, 256, 0, ctx->stream>>>(key[c], n_host, n_dev, shift, ctx->d.hist, nblocks);
+        k_sort_scan<<<1, 1024, 0, ctx->stream>>>(ctx->d.hist, 256 * nblocks);
+        k_sort_scatter<<<nblocks, SORT_THREADS, 0, ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host,
+                                                                  n_dev, shift, ctx->d.hist, nblocks);
+        ctx->launches += 3;
+        c ^= 1;
+    }
+    *cur = c;
+}
+
+// ------------------------------------------------------------------------------------------
+// SoA gather into sorted order
+// ------------------------------------------------------------------------------------------
+__global__ void k_gather(Dev d) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    int o = d.perm[i];
+    for (int a = 0; a < 3; ++a) {
+        d.sx[a][i] = (a < d.D) ? d.x[a][o] : 0.0;
+        d.sv[a][i] = (a < d.D) ? d.v[a][o] : 0.0;
+    }
+    d.sm[i] = d.m[o];
+    d.srho[i] = d.rho[o];
+    d.su[i] = d.u[o];
+    d.sh[i] = d.h[o];
+    d.smat[i] = d.mat[o];
+    if (d.flags & SPH_F_SOLID)
+        for (int k = 0; k < 6; ++k) d.sS[k][i] = d.S[k][o];
+    if (d.flags & SPH_F_DAMAGE) d.sdmg[i] = d.dmg[o];
+}
+
+void sph_stage_order(sph_ctx *ctx) {
+    Dev &d = ctx->d;
+    const int n = d.n;
+    int nb = min(sph_ceil_div(n, 256), 1024);
+    k_bbox_partial<<<nb, 256, 0, ctx->stream>>>(d, nb);
+    k_bbox_final<<<1, 32, 0, ctx->stream>>>(d, nb);
+    k_keys<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
+    ctx->launches += 3;
+    int cur = 0;
+    sph_radix_sort(ctx, d.key, d.idx, n, nullptr, d.D * d.L, &cur);
+    d.keys = d.key[cur];
+    d.perm = d.idx[cur];
+    ctx->sort_cur = cur;
+    k_gather<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
+    ctx->launches += 1;
+}

@@ -1,0 +1,121 @@
+// Internal declarations shared by the CUDA translation units of libsph_b200.so.
+// (Nothing here is shared with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/sph.h"
+
+typedef unsigned long long u64;
+typedef long long i64;
+
+#define SPH_MAX_MAT 16
+#define SPH_WARP 32
+
+// Device-side status block (one per context, in the workspace).
+struct DevStatus {
+    int n_nodes;        // internal octree nodes found by the last build
+    int err_nb_overflow;
+    int err_stack;
+    int nb_max;         // largest partner count seen
+    int pad[4];
+};
+
+// Root cube of the last build (device).
+struct DevRoot {
+    double xmin[3];
+    double s0;
+    double scale;       // 2^L / s0
+    double pad[3];
+};
+
+struct Mats {
+    sph_material m[SPH_MAX_MAT];
+};
+
+// All device pointers of one context. Passed by value to kernels (plain POD).
+struct Dev {
+    int D, L, flags, cap;       // cap = max_neighbours
+    int n;
+    int n_des;
+    double theta2, G, eps2, av_alpha, av_beta, av_eps;
+    // ---- master state, original order ----
+    double *x[3], *v[3], *m, *rho, *u, *S[6], *dmg, *h;
+    int *mat, *n_act;
+    i64 *flaw_off;
+    double *flaw_eps;
+    // ---- RK2 base copy (x v rho u S dmg: 15 arrays contiguous) ----
+    double *q0;
+    // ---- sorted working copies ----
+    double *sx[3], *sv[3], *sm, *srho, *su, *sS[6], *sdmg, *sh;
+    int *smat;
+    // ---- order ----
+    u64 *key[2];
+    int *idx[2];                // idx[cur][i] = original index of sorted i (perm)
+    u64 *keys;                  // sorted keys (alias of key[cur] after the sort)
+    int *perm;                  // alias of idx[cur]
+    unsigned *hist;             // radix histograms
+    double *partial;            // bbox partials
+    DevRoot *root;
+    DevStatus *status;
+    // ---- tree (depth-first order) ----
+    u64 *nkey[2];
+    int *nhi[2];
+    int *nlevel, *nlo, *nhi_s;  // per node
+    int *nskip;                 // first node after the subtree (pre-order)
+    int *child;                 // NC per node: >=0 node, -1 empty, -2 leaf
+    int *child_lo;              // NC+1 per node
+    double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
+    // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
+    int *nb;
+    int *nb_cnt;
+    int *own_cnt;               // n_a of eq. 73
+    // ---- pre-pass ----
+    double *p, *cs, *vol, *sr2[6];      // pressure, sound speed, m/rho, sigma/rho^2
+    // ---- rates, sorted order ----
+    double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *strain;
+    int *n_act_new;
+    // ---- staging ----
+    double *stage;              // n doubles, for unsorting downloads
+    int *stage_i;               // n ints
+};
+
+struct sph_ctx {
+    sph_config cfg;
+    Dev d;
+    Mats mats;
+    cudaStream_t stream;
+    void *ws;
+    size_t ws_bytes;
+    int have_state, have_tree, have_lists, have_rates;
+    i64 launches;
+    int sort_cur;
+    char err[512];
+};
+
+#define SPH_LAUNCH(ctx) ((ctx)->launches++)
+
+static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
+
+// ---- sort.cu ----
+// LSD radix sort of (key, val) pairs, `bits` low key bits significant. n is read on the host
+// (n_host) or, if n_dev != NULL, from device memory (kernels early-exit; grids sized for n_host).
+// Result ends in key[*cur], val[*cur].
+void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur);
+
+// ---- per-stage entry points (each enqueues kernels on ctx->stream) ----
+void sph_stage_order(sph_ctx *ctx);     // A1 + A2
+void sph_stage_tree(sph_ctx *ctx);      // A3 + A4
+void sph_stage_neigh(sph_ctx *ctx);     // A5
+void sph_stage_rhs(sph_ctx *ctx);       // A6-A10
+void sph_stage_gravity(sph_ctx *ctx);   // A11
+void sph_stage_update(sph_ctx *ctx, double c, int commit);   // A12 (one of the two updates)
+void sph_stage_writeback_h(sph_ctx *ctx);
+
+// ---- exact-order arithmetic for the floating-point decisions (never contracted to FMA) ----
+__device__ __forceinline__ double sph_r2_exact(double dx, double dy, double dz, int D) {
+    double r2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+    if (D == 3) r2 = __dadd_rn(r2, __dmul_rn(dz, dz));
+    return r2;
+}

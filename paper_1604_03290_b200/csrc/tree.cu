@@ -1,0 +1,174 @@
+// A3 + A4: octree topology from the sorted Morton keys, then pseudo-particles bottom-up.
+//
+// The tree is the paper's Barnes-Hut octree (cubic cells, 2^D
+// sub-cells, one particle per leaf) without the chains of single-child cells its insertion
+// creates (reading U14).  An internal node is a cell in which two particles that are
+// adjacent in Morton order first separate.  Instead of the paper's lock-based top-down insertion
+// every node is found independently from the sorted keys:
+//   k_find_nodes : one thread per adjacent pair; binary search for the start of the pair's cell;
+//                  the pair that closes the FIRST occupied sub-cell emits the node (lo, level, hi)
+//   radix sort   : nodes sorted by (lo, level)  == depth-first (pre-order) numbering
+//   k_fill_nodes : child boundaries by binary search in the node's key range; child node ids by
+//                  binary search in the sorted node keys
+//   k_moments    : one launch per level, deepest first: mass, centre of mass (monopole only,
+//                  PAPER.md:370, :380, :473-475), tight bounding box and hmax.  Children are
+//                  summed in octant order, every operation rounded separately (reading U15), so
+//                  that the opening decisions of the gravity walk are reproducible bit for bit.
+#include "sph_internal.cuh"
+
+__device__ __forceinline__ int lower_bound_key(const u64 *__restrict__ k, int lo, int hi, u64 v) {
+    while (lo < hi) {   // first index in [lo,hi) with k[i] >= v
+        int mid = (lo + hi) >> 1;
+        if (k[mid] < v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void k_find_nodes(Dev d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int DL = d.D * d.L;
+    bool emit = false;
+    u64 nk = 0;
+    int hi = 0;
+    if (i < d.n - 1) {
+        const u64 ka = d.keys[i], kb = d.keys[i + 1];
+        const u64 x = ka ^ kb;
+        if (x != 0) {
+            const int common = DL - (64 - __clzll((long long)x));   // common leading bits of the DL-bit keys
+            const int lvl = common / d.D;
+            const int shift = d.D * (d.L - lvl);                    // low bits below the cell prefix
+            int lo;
+            u64 cell0;
+            if (lvl == 0) { lo = 0; cell0 = 0; }
+            else {
+                cell0 = (ka >> shift) << shift;
+                lo = lower_bound_key(d.keys, 0, i, cell0);
+            }
+            // representative pair: i closes the first occupied sub-cell of the node
+            if ((d.keys[lo] >> (shift - d.D)) == (ka >> (shift - d.D))) {
+                emit = true;
+                hi = (lvl == 0) ? d.n : lower_bound_key(d.keys, i + 1, d.n, cell0 + (1ull << shift));
+                nk = ((u64)lo << 8) | (u64)lvl;
+            }
+        }
+    }
+    unsigned m = __ballot_sync(0xffffffffu, emit);
+    if (m) {
+        int lane = threadIdx.x & 31, base = 0;
+        if (lane == __ffs(m) - 1) base = atomicAdd(&d.status->n_nodes, __popc(m));
+        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+        if (emit) {
+            int slot = base + __popc(m & ((1u << lane) - 1u));
+            d.nkey[0][slot] = nk;
+            d.nhi[0][slot] = hi;
+        }
+    }
+}
+
+__global__ void k_fill_nodes(Dev d, const u64 *__restrict__ nkey, const int *__restrict__ nhi) {
+    const int nd = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nn = d.status->n_nodes;
+    if (nd >= nn) return;
+    const int D = d.D, NC = 1 << D;
+    const u64 nk = nkey[nd];
+    const int lo = (int)(nk >> 8), lvl = (int)(nk & 255u), hi = nhi[nd];
+    d.nlo[nd] = lo; d.nhi_s[nd] = hi; d.nlevel[nd] = lvl;
+    const double s = ldexp(d.root->s0, -lvl);               // eq. 68 (exact)
+    d.ns2[nd] = __dmul_rn(s, s);
+    {   // skip index: first node whose range starts at or after hi (nodes are sorted by (lo, level))
+        const u64 want = (u64)hi << 8;
+        int l2 = nd + 1, h2 = nn;
+        while (l2 < h2) { int mid = (l2 + h2) >> 1; if (nkey[mid] < want) l2 = mid + 1; else h2 = mid; }
+        d.nskip[nd] = l2;
+    }
+    const int shift = D * (d.L - lvl);
+    const u64 prefix = (lvl == 0) ? 0ull : (d.keys[lo] >> shift);
+    int b = lo;
+    int *cl = d.child_lo + (size_t)nd * (NC + 1);
+    int *ch = d.child + (size_t)nd * NC;
+    cl[0] = lo;
+    for (int c = 0; c < NC; ++c) {
+        int e = (c == NC - 1) ? hi : lower_bound_key(d.keys, b, hi, ((prefix << D) | (u64)(c + 1)) << (shift - D));
+        cl[c + 1] = e;
+        int code;
+        if (e == b) code = -1;
+        else if (e - b == 1 || d.keys[b] == d.keys[e - 1]) code = -2;
+        else {
+            u64 x = d.keys[b] ^ d.keys[e - 1];
+            int common = D * d.L - (64 - __clzll((long long)x));
+            int clvl = common / D;
+            u64 want = ((u64)b << 8) | (u64)clvl;
+            int l2 = nd + 1, h2 = nn;                       // children follow their parent in pre-order
+            while (l2 < h2) { int mid = (l2 + h2) >> 1; if (nkey[mid] < want) l2 = mid + 1; else h2 = mid; }
+            code = l2;
+        }
+        ch[c] = code;
+        b = e;
+    }
+}
+
+__global__ void k_moments(Dev d, int level) {
+    const int nd = blockIdx.x * blockDim.x + threadIdx.x;
+    if (nd >= d.status->n_nodes) return;
+    if (d.nlevel[nd] != level) return;
+    const int D = d.D, NC = 1 << D;
+    const int *cl = d.child_lo + (size_t)nd * (NC + 1);
+    const int *ch = d.child + (size_t)nd * NC;
+    double M = 0.0, S[3] = {0, 0, 0};
+    double bmin[3] = {INFINITY, INFINITY, INFINITY}, bmax[3] = {-INFINITY, -INFINITY, -INFINITY}, hmax = 0.0;
+    for (int c = 0; c < NC; ++c) {
+        const int code = ch[c];
+        if (code == -1) continue;
+        if (code >= 0) {
+            const double mc = d.nmass[code];
+            M = __dadd_rn(M, mc);
+            for (int a = 0; a < D; ++a) {
+                S[a] = __dadd_rn(S[a], __dmul_rn(mc, d.ncom[a][code]));
+                bmin[a] = fmin(bmin[a], d.nbmin[a][code]);
+                bmax[a] = fmax(bmax[a], d.nbmax[a][code]);
+            }
+            hmax = fmax(hmax, d.nhmax[code]);
+        } else {
+            for (int p = cl[c]; p < cl[c + 1]; ++p) {
+                const double mp = d.sm[p];
+                M = __dadd_rn(M, mp);
+                for (int a = 0; a < D; ++a) {
+                    const double xp = d.sx[a][p];
+                    S[a] = __dadd_rn(S[a], __dmul_rn(mp, xp));
+                    bmin[a] = fmin(bmin[a], xp);
+                    bmax[a] = fmax(bmax[a], xp);
+                }
+                hmax = fmax(hmax, d.sh[p]);
+            }
+        }
+    }
+    d.nmass[nd] = M;
+    for (int a = 0; a < 3; ++a) {
+        d.ncom[a][nd] = (a < D) ? __ddiv_rn(S[a], M) : 0.0;
+        d.nbmin[a][nd] = (a < D) ? bmin[a] : 0.0;
+        d.nbmax[a][nd] = (a < D) ? bmax[a] : 0.0;
+    }
+    d.nhmax[nd] = hmax;
+}
+
+__global__ void k_zero_status(Dev d) {
+    d.status->n_nodes = 0;
+}
+
+void sph_stage_tree(sph_ctx *ctx) {
+    Dev &d = ctx->d;
+    const int n = d.n;
+    k_zero_status<<<1, 1, 0, ctx->stream>>>(d);
+    k_find_nodes<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
+    ctx->launches += 2;
+    int bits = 8, t = n;
+    while (t > 0) { ++bits; t >>= 1; }
+    int cur = 0;
+    sph_radix_sort(ctx, d.nkey, d.nhi, n, &d.status->n_nodes, bits, &cur);
+    k_fill_nodes<<<sph_ceil_div(n, 128), 128, 0, ctx->stream>>>(d, d.nkey[cur], d.nhi[cur]);
+    ctx->launches += 1;
+    for (int lvl = d.L - 1; lvl >= 0; --lvl) {
+        k_moments<<<sph_ceil_div(n, 128), 128, 0, ctx->stream>>>(d, lvl);
+        ctx->launches += 1;
+    }
+}

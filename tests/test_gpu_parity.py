@@ -1,0 +1,304 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the CPU oracle on the same
+seeded inputs.  Bars (BASELINE.json north_star):
+  * Morton keys, permutation, tree topology, node moments, neighbour sets: bit-exact;
+  * every FP64 rate: per particle |g - o| <= 1e-10 |o|  or  |g - o| <= 1e-13 * A, A = the oracle's sum
+    of absolute pair contributions (reading T1: where the pair terms cancel the relative error of
+    the sum is meaningless; FP64 re-ordering error is bounded by n * 1.1e-16 * A);
+  * n_act (an integer decided by a floating-point comparison strain >= threshold): exact except
+    where a threshold lies within 1e-12 relative of the oracle's strain.
+"""
+import numpy as np
+import pytest
+
+import sph_inputs
+from oracle import oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+REL, ABS_A = 1e-10, 1e-13
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_1604_03290_b200 as P
+    from paper_1604_03290_b200 import build
+    build.build()
+    return P
+
+
+def make_ctx(P, w, **kw):
+    cfg, mats = P.config_of(w, **kw)
+    ctx = P.sph_create(cfg, mats)
+    ctx.upload_workload(w)
+    return ctx
+
+
+def assert_close(name, g, o, A=None, rel=REL, abs_a=ABS_A, floor=0.0):
+    g, o = np.asarray(g, dtype=np.float64), np.asarray(o, dtype=np.float64)
+    assert g.shape == o.shape, (name, g.shape, o.shape)
+    err = np.abs(g - o)
+    ok = err <= rel * np.abs(o) + floor
+    if A is not None:
+        ok |= err <= abs_a * np.asarray(A)
+    assert np.all(np.isfinite(g)), f"{name}: non-finite GPU values"
+    if not ok.all():
+        bad = np.flatnonzero(~ok.reshape(-1))
+        k = bad[np.argmax(err.reshape(-1)[bad])]
+        raise AssertionError(f"{name}: {bad.size}/{g.size} outside tolerance; worst flat index {k}: "
+                             f"gpu {g.reshape(-1)[k]!r} oracle {o.reshape(-1)[k]!r} "
+                             f"A {None if A is None else np.asarray(A).reshape(-1)[k]!r}")
+
+
+def canonical(nodes):
+    order = np.lexsort((nodes["prefix"], nodes["level"]))
+    return {k: v[order] for k, v in nodes.items()}
+
+
+def check_order_and_tree(P, ctx, w, h=None):
+    tree = orc.Tree(w, h=h)
+    okey, operm = tree.order()
+    keys, perm, root = ctx.get_order()
+    assert np.array_equal(keys, okey), "Morton keys differ"
+    assert np.array_equal(perm, operm), "permutation differs"
+    assert root[3] == tree.s0
+    on = tree.nodes()
+    gn = canonical(ctx.get_tree())
+    assert gn["level"].size == on["level"].size, "node count differs"
+    for k in ("level", "prefix", "lo", "hi"):
+        assert np.array_equal(gn[k], on[k]), f"tree {k} differs"
+    # moments: octant-order, unfused arithmetic on both sides (reading U15) -> identical bits
+    for k in ("mass", "com", "bmin", "bmax", "hmax"):
+        g, o = gn[k], on[k]
+        if k in ("com", "bmin", "bmax"):
+            g, o = g[:, :w.dim], o[:, :w.dim]
+        assert np.array_equal(g, o), f"node {k} differs (max rel {np.max(np.abs(g - o) / np.abs(o).clip(1e-300))})"
+    return tree
+
+
+def check_neighbours(ctx, off_o, idx_o):
+    off, idx = ctx.get_neighbours()
+    assert np.array_equal(off, off_o), "partner counts differ"
+    assert np.array_equal(idx, idx_o), "partner sets differ"
+
+
+def check_rates(w, g, o, targets=None):
+    t = slice(None) if targets is None else targets
+    assert_close("p", g["p"][t], o["p"], rel=1e-12)
+    assert_close("cs", g["cs"][t], o["cs"], rel=1e-13)
+    assert_close("drho", g["drho"][t], o["drho"], o["A_drho"])
+    assert_close("du", g["du"][t], o["du"], o["A_du"])
+    assert_close("dv", g["dv"][:, t], o["dv"], o["A_dv"])
+    if w.flags & orc.F_SOLID:
+        assert_close("dS", g["dS"][:, t], o["dS"], o["A_dS"])
+    if w.flags & orc.F_GRAVITY:
+        assert_close("ag", g["ag"][:, t], o["ag"], o["A_ag"])
+    if w.flags & orc.F_DENSITY_SUM:
+        assert_close("rho", g["rho"][t], o["rho"][t], rel=1e-12)
+    if w.flags & orc.F_DAMAGE:
+        # strain = sigma_max / ((1 - d) E): the eigenvalue carries an error relative to |sigma|, not to itself
+        tt = np.arange(w.n)[t]
+        K = np.array([m["tA"] if m["eos"] == 2 else m["K0"] for m in w.materials])[w.mat[tt]]
+        mu = np.array([m["mu"] for m in w.materials])[w.mat[tt]]
+        E = 9.0 * K * mu / np.maximum(3.0 * K + mu, 1e-300)
+        d3 = w.dmg[tt] ** 3
+        floor = 1e-13 * np.abs(o["sigma"]).max(axis=0) / np.maximum((1.0 - d3) * E, 1e-300)
+        assert_close("strain", g["strain"][t], o["strain"], rel=1e-10, floor=np.where(np.isfinite(floor), floor, 0.0))
+        na_g, na_o = g["n_act_new"][t], o["n_act"]
+        diff = np.flatnonzero(na_g != na_o)
+        for k in diff:       # allowed only in the tie zone of the threshold comparison
+            a = tt[k]
+            eps = w.flaw_eps[w.flaw_off[a]:w.flaw_off[a + 1]]
+            s = o["strain"][k]
+            assert np.any(np.abs(eps - s) <= 1e-12 * abs(s)), f"n_act differs at particle {a} away from a tie"
+        same = na_g == na_o
+        assert_close("ddmg", g["ddmg"][t][same], o["ddmg"][same], rel=1e-10)
+
+
+CASES = {
+    "C1-twin": lambda: sph_inputs.make("C1", scale=0.25, twin=True),
+    "C1-nominal": lambda: sph_inputs.make("C1", scale=0.25),
+    "C2-twin": lambda: sph_inputs.c2_gas_sphere(n=3000, twin=True),
+    "C3-twin": lambda: sph_inputs.make("C3", scale=0.006, twin=True),
+    "C4-twin": lambda: sph_inputs.make("C4", scale=0.002, twin=True),
+    "C5-twin": lambda: sph_inputs.make("C5", scale=0.001, twin=True),
+    "blob3d": lambda: sph_inputs.random_blob(2500, dim=3, seed=3, duplicates=7),
+    "blob2d": lambda: sph_inputs.random_blob(1500, dim=2, seed=4, duplicates=5),
+    "blob3d-varh": lambda: sph_inputs.random_blob(2000, dim=3, seed=5, variable_h=True),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_full_evaluation_parity_small(P, name):
+    """Sizes the O(N^2) oracle finishes in seconds; several 32-particle groups, tiles and a ragged tail."""
+    w = CASES[name]()
+    assert w.n % 32 != 0 or name.startswith("blob")
+    ctx = make_ctx(P, w, h_iters=0)
+    ctx.evaluate()
+    ctx.sync()
+    check_order_and_tree(P, ctx, w)
+    o = orc.evaluate(w, mode="brute", h_iters=0)
+    check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    g = ctx.download()
+    assert np.array_equal(g["nb_count"], np.diff(o["nb_off"]))
+    check_rates(w, g, o)
+    # purity: an evaluation never changes x, v, u, S, dmg, n_act (rho only under DENSITY_SUM)
+    for k in ("x", "v", "u", "S", "dmg"):
+        assert np.array_equal(g[k], getattr(w, k)), k
+    assert np.array_equal(g["n_act"], w.n_act)
+    if not (w.flags & orc.F_DENSITY_SUM):
+        assert np.array_equal(g["rho"], w.rho)
+    assert ctx.launch_count() > 0
+    ctx.close()
+
+
+def test_separate_calls_equal_evaluate(P):
+    w = CASES["blob3d"]()
+    a = make_ctx(P, w)
+    a.evaluate()
+    ga = a.download(P.RATE_FIELDS)
+    b = make_ctx(P, w)
+    b.build_tree(); b.find_neighbours(); b.gravity(); b.rhs()
+    gb = b.download(P.RATE_FIELDS)
+    for k in ga:
+        assert np.array_equal(ga[k], gb[k]), k
+    # determinism: a second evaluation on the same context returns identical bits
+    a.evaluate()
+    gc = a.download(P.RATE_FIELDS)
+    for k in ga:
+        assert np.array_equal(ga[k], gc[k]), k
+
+
+def test_variable_h_update_eq73(P):
+    """eq. 73 inside sph_find_neighbours (h_iters = 1): n_a by own h, new h, symmetric partner sets."""
+    w = sph_inputs.c2_gas_sphere(n=2500)
+    w.h = w.h * np.random.default_rng(1).uniform(0.85, 1.2, w.n)      # un-converge
+    ctx = make_ctx(P, w, h_iters=1)
+    ctx.evaluate()
+    g = ctx.download()
+    o = orc.evaluate(w, mode="brute", h_iters=1)
+    assert_close("h", g["h"], o["h"], rel=4e-16)                     # cbrt may differ by an ulp (reading U5)
+    if np.array_equal(g["h"], o["h"]):
+        check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    else:                                                            # same sets unless a pair sits on the rim
+        w2 = w.copy(); w2.h = g["h"]
+        off, idx = orc.neighbours(w2, mode="brute")
+        check_neighbours(ctx, off, idx)
+    check_rates(w, g, o)
+
+
+def test_device_resident_upload_and_download(P):
+    import torch
+    w = CASES["blob3d"]()
+    cfg, mats = P.config_of(w)
+    ctx = P.sph_create(cfg, mats)
+    dev = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).cuda()
+    ctx.upload(x=dev(w.x, torch.float64), v=dev(w.v, torch.float64), m=dev(w.m, torch.float64),
+               rho=dev(w.rho, torch.float64), u=dev(w.u, torch.float64), S=dev(w.S, torch.float64),
+               dmg=dev(w.dmg, torch.float64), h=dev(w.h, torch.float64), mat=dev(w.mat, torch.int32),
+               n_act=dev(w.n_act, torch.int32), flaw_off=dev(w.flaw_off, torch.int64),
+               flaw_eps=dev(w.flaw_eps, torch.float64), device=True)
+    ctx.evaluate()
+    gd = ctx.download(device=True)
+    ctx.sync()
+    ref = make_ctx(P, w)
+    ref.evaluate()
+    gh = ref.download()
+    for k in gh:
+        assert np.array_equal(gd[k].cpu().numpy(), gh[k]), k
+
+
+@pytest.mark.parametrize("name", ["C1-twin", "C4-twin", "C2-twin"])
+def test_step_parity(P, name):
+    """sph_step = two complete evaluations + two updates (eqs. 52-53).  Per-evaluation parity is the
+    contract; the trajectory after a step is compared with a looser bound (rates enter multiplied by dt)."""
+    w = CASES[name]()
+    ctx = make_ctx(P, w, h_iters=0)
+    ctx.step(w.dt)
+    g = ctx.download()
+    w0 = w.copy(); w0.h_iters = 0
+    qn, f1, f2 = orc.step(w0, w.dt, mode="brute")
+    for k in ("x", "v", "rho", "u", "S", "dmg"):
+        go, oo = g[k], getattr(qn, k)
+        scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
+        assert np.all(np.abs(go - oo) <= 1e-9 * np.abs(oo) + 1e-12 * scale), k
+    assert np.mean(g["n_act"] == qn.n_act) > 0.999
+    # the rates left in the context are those of the second evaluation (at the predicted state)
+    assert_close("dv(step)", g["dv"], f2["dv"], f2["A_dv"], rel=1e-8, abs_a=1e-11)
+    # multi-step protocol: download the GPU state, hand it to the oracle, compare that evaluation
+    w1 = w.copy()
+    for k in ("x", "v", "rho", "u", "S", "dmg", "h", "n_act"):
+        setattr(w1, k, g[k].copy())
+    ctx.evaluate()
+    g1 = ctx.download()
+    o1 = orc.evaluate(w1, mode="brute", h_iters=0)
+    check_neighbours(ctx, o1["nb_off"], o1["nb_idx"])
+    check_rates(w1, g1, o1)
+
+
+def test_degenerate_inputs(P):
+    # one particle; two particles; all particles coincident; no partners at all; 2-D line
+    base = sph_inputs.random_blob(64, dim=3, seed=9)
+    for idx in ([0], [0, 1], list(range(33))):
+        w = base.subset(idx)
+        ctx = make_ctx(P, w)
+        ctx.evaluate()
+        g = ctx.download()
+        o = orc.evaluate(w, mode="brute")
+        check_order_and_tree(P, ctx, w)
+        check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+        check_rates(w, g, o)
+    w = base.copy()
+    w.x[:] = w.x[:, :1]                                  # all coincident: one multi-particle leaf, no node
+    ctx = make_ctx(P, w)
+    ctx.evaluate()
+    g = ctx.download()
+    o = orc.evaluate(w, mode="brute")
+    assert ctx.get_tree()["level"].size == 0
+    check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    check_rates(w, g, o)
+    w = base.copy()
+    w.h[:] = 1e-6                                        # nobody has partners: every sum is empty
+    ctx = make_ctx(P, w)
+    ctx.evaluate()
+    g = ctx.download()
+    assert g["nb_count"].sum() == 0
+    for k in ("drho", "du", "dv", "dS"):
+        assert not g[k].any()
+    o = orc.evaluate(w, mode="brute")
+    check_rates(w, g, o)
+
+
+def test_error_paths(P):
+    w = CASES["blob3d"]()
+    cfg, mats = P.config_of(w)
+    ctx = P.sph_create(cfg, mats)
+    with pytest.raises(P.SphError) as e:
+        ctx.build_tree()                                 # nothing uploaded yet
+    assert e.value.code == P.SPH_ERR_STATE
+    ctx.upload_workload(w)
+    with pytest.raises(P.SphError) as e:
+        ctx.rhs()
+    assert e.value.code == P.SPH_ERR_STATE
+    with pytest.raises(P.SphError) as e:
+        ctx.gravity()
+    assert e.value.code == P.SPH_ERR_STATE
+    ctx.build_tree()
+    with pytest.raises(P.SphError) as e:
+        ctx.rhs()
+    assert e.value.code == P.SPH_ERR_STATE
+    ctx.close()
+    # interaction list capacity (the paper's interactionsList is a fixed array too)
+    ctx = make_ctx(P, w, max_neighbours=8)
+    ctx.build_tree(); ctx.find_neighbours()
+    with pytest.raises(P.SphError) as e:
+        ctx.sync()
+    assert e.value.code == P.SPH_ERR_NEIGHBOUR_OVERFLOW
+    ctx.close()
+    # misaligned / short workspace
+    import ctypes as C
+    import torch
+    L = P.load_library()
+    buf = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    assert L.sph_create(C.byref(cfg), mats, C.c_void_p(buf.data_ptr()), 1 << 20, None, C.byref(h)) == P.SPH_ERR_WORKSPACE
+    assert L.sph_create(C.byref(cfg), mats, C.c_void_p(buf.data_ptr() + 8), 1 << 40, None, C.byref(h)) == P.SPH_ERR_WORKSPACE
