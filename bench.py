@@ -1,0 +1,418 @@
+"""bench.py -- throughput of the whole hot path on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1..C5] [--impl ours|reference]
+
+A "step" is one sph_step (eqs. 52-53): TWO complete right-hand-side evaluations
+(Morton order, octree, pseudo-particles, interaction partners, SPH sums, self-gravity; the sub-step
+list of PAPER.md:693) and two updates.  metric = particle-updates/s = N * RHS evaluations / time
+(SURVEY.md 8(d)).  Prints ONE JSON line (contract in DESIGN.md "Measurement").
+
+  value         device-resident state, CUDA-event time of exactly K steps, max over ranks
+  e2e           the same step through the C ABI with HOST buffers: sph_upload (pinned host state) ->
+                sph_step -> sph_download (host state) inside the timed region
+  roofline      dominant kernel of the step, timed live by the library's CUDA-event stage brackets
+  cpu_baseline  the CPU oracle (oracle/, tree mode, as it stands) on a bounded sample, rank 0, N=1
+  --impl reference   the oracle alone, same metric/config (there is no upstream code: PAPER.md only)
+
+Multi-GPU: the path is single-GPU by north_star ("one GPU only"); --gpus N runs N independent
+replicas (replicas only, no data-path collective), weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import sph_inputs  # noqa: E402
+
+METRIC = "particle-updates/s (full FP64 SPH RHS incl. tree gravity); % FP64/HBM roofline"
+UNIT = "particle-updates/s"
+DEFAULT_WORKLOAD = "C5"
+L2_BYTES = 126 << 20
+# algorithmic FP64 flop per unit (add = mul = cmp = 1, fma = 2, div = sqrt = 1)
+FLOP_PER_INTERACTION = 20.0     # eq. 51: 3 sub, 5 for r^2, +eps^2, sqrt, mul, div, 3 fma (6), G*M
+FLOP_PER_OPENING_TEST = 11.0    # eq. 50: 3 sub, 5 for r^2, theta^2 * r^2, compare, (s^2 precomputed)
+FLOP_PER_PAIR = {(3, True): 130.0, (2, True): 80.0, (3, False): 60.0, (2, False): 45.0}
+
+
+def _peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written) for HBM; FP64 is measured live."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.t = threading.Thread(target=self._read, daemon=True)
+        self.t.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except ValueError:
+                continue
+            for k, name in enumerate(names):
+                if r[5 + k].lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic work per stage
+# ---------------------------------------------------------------------------------------------
+def stage_work(stage, w, counters, evals):
+    """(bound, unit, amount per evaluation) of one stage: algorithmic bytes or flops, NOT traffic."""
+    n, D = w.n, w.dim
+    solid = bool(w.flags & sph_inputs.F_SOLID)
+    damage = bool(w.flags & sph_inputs.F_DAMAGE)
+    nstate = 2 * D + 4 + (6 if solid else 0) + (1 if damage else 0)      # doubles moved by the reorder
+    passes = (D * 21 + 7) // 8
+    if stage == "gravity":
+        return "alu", "TFLOP/s", FLOP_PER_INTERACTION * counters["n_inter"] + FLOP_PER_OPENING_TEST * counters["n_visit"]
+    if stage == "pairs":
+        return "alu", "TFLOP/s", FLOP_PER_PAIR[(D, solid)] * counters["n_pairs"]
+    if stage == "density":
+        return "alu", "TFLOP/s", 30.0 * counters["n_pairs"]
+    by = {"keys": 8 * D * 2 + 12,                       # bbox read + key pass read, key + index written
+          "sort": passes * 24,                          # (key, index) read + written per 8-bit pass
+          "reorder": nstate * 16 + 12,                  # every state array read + written, perm + mat
+          "tree": 8 + counters["n_nodes"] / max(n, 1) * (12 + 4 * (2 * (1 << D) + 1) + 24),
+          "moments": counters["n_nodes"] / max(n, 1) * (8 * (4 + 2 * D + 1) + 4 * (2 * (1 << D) + 1)) + 8 * (D + 2),
+          "neighbours": 4 * counters["n_pairs"] / max(n, 1) + 8 * (D + 1) + 4,
+          "prepass": 8 * (3 + (6 if solid else 0) + (1 if damage else 0)) + 4 + 8 * 9,
+          "update": 3 * 8 * 15}[stage]
+    return "hbm", "GB/s", float(by) * n
+
+
+def run_ours(args, rank, world):
+    import torch
+    import paper_1604_03290_b200 as P
+    from paper_1604_03290_b200 import build as sph_build
+
+    sph_build.build()                       # fails loudly if nvcc or the sources are missing: no fallback
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", rank))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    t_gen = time.time()
+    w = sph_inputs.make(args.workload, scale=args.scale, seed=sph_inputs_seed(args.workload) + rank)
+    t_gen = time.time() - t_gen
+    cfg, mats = P.config_of(w)
+    ctx = P.sph_create(cfg, mats, device=dev)
+    ctx.upload_workload(w)
+    ws_bytes = ctx.workspace_bytes
+    small = ws_bytes < 4 * L2_BYTES       # working set may sit in the 126 MB L2: flush between steps
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if small else None
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            torch.distributed.barrier()
+
+    # ---- device-resident arm ----
+    for _ in range(args.warmup):
+        ctx.step(w.dt)
+    ctx.sync()
+    ctx.timing_enable(True)
+    ctx.timing_read()
+    launches0 = ctx.launch_count()
+    sampler = ClockSampler(local)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    sampler.start()
+    for k in range(args.steps):
+        if flush is not None:
+            flush.fill_(k & 1)
+        ev[k][0].record()
+        ctx.step(w.dt)
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    ctx.sync()
+    if flush is not None:
+        ms_dev = sum(a.elapsed_time(b) for a, b in ev)
+    else:
+        ms_dev = ev[0][0].elapsed_time(ev[-1][1])
+    launches = ctx.launch_count() - launches0
+    stages = ctx.timing_read()
+    ctx.timing_enable(False)
+    counters = ctx.get_counters()
+
+    # ---- end-to-end arm: host buffers through the C ABI every step ----
+    e2e_steps = max(1, min(args.steps, 3))
+    n = w.n
+    pin = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=True)
+    host = dict(x=pin((3, n), torch.float64), v=pin((3, n), torch.float64), rho=pin((n,), torch.float64),
+                u=pin((n,), torch.float64), S=pin((6, n), torch.float64), dmg=pin((n,), torch.float64),
+                h=pin((n,), torch.float64), n_act=pin((n,), torch.int32))
+    const = dict(m=pin((n,), torch.float64), mat=pin((n,), torch.int32))
+    const["m"].numpy()[:] = w.m
+    const["mat"].numpy()[:] = w.mat
+    ctx.download(tuple(host), out=host)                     # current state -> host (untimed)
+    h2d = sum(t.numel() * t.element_size() for t in list(host.values()) + list(const.values()))
+    d2h = sum(t.numel() * t.element_size() for t in host.values())
+    if w.dim == 2:
+        h2d -= 2 * n * 8                                    # z rows of x and v are not copied in 2-D
+
+    def e2e_step():
+        ctx.upload(device=False, **host, **const)
+        ctx.step(w.dt)
+        ctx.download(tuple(host), out=host)                 # synchronises (host destination)
+
+    e2e_step()                                              # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    ms_e2e = (time.perf_counter() - t0) * 1e3 / e2e_steps
+
+    fp64_peak = P.sph_measure_fp64_peak()
+    ctx.close()
+    return dict(w=w, ms_dev=ms_dev, launches=launches, stages=stages, counters=counters, clocks=clocks,
+                ms_e2e=ms_e2e, h2d=h2d, d2h=d2h, fp64_peak=fp64_peak, l2_flush=small, ws_bytes=ws_bytes,
+                t_gen=t_gen)
+
+
+def sph_inputs_seed(name):
+    return {"C1": 1604, "C2": 1605, "C3": 1606, "C4": 1607, "C5": 1608}[name]
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle arm (test infrastructure timed as a baseline; never on the product path)
+# ---------------------------------------------------------------------------------------------
+def oracle_time(w, budget_s=20.0):
+    """Time the oracle (tree mode, as it stands, OpenMP on the host cores) on one complete RHS
+    evaluation of workload `w`.  Small workloads are evaluated whole.  Large ones on a bounded
+    sample: the evaluation is run for M1 and M2 target particles (the tree and the per-particle
+    pre-pass always cover all N particles), and  T(N) = T_fixed + N * t_per  is formed from the two.
+    Returns (seconds per complete evaluation, description of the sample)."""
+    from oracle import oracle as orc
+    n = w.n
+    orc.lib()
+    if n <= 100_000:
+        t0 = time.perf_counter()
+        orc.evaluate(w, mode="tree")
+        t = time.perf_counter() - t0
+        return t, f"one complete RHS evaluation of all {n} particles (oracle tree mode)"
+    rng = np.random.default_rng(12345)
+    m1 = 2000
+    t1s = np.sort(rng.choice(n, m1, replace=False))
+    t0 = time.perf_counter()
+    orc.evaluate(w, mode="tree", targets=t1s)
+    T1 = time.perf_counter() - t0
+    # choose M2 so that the second run takes about the budget
+    m2 = int(min(n // 2, max(4 * m1, m1 * budget_s / max(T1 * 0.2, 1e-3))))
+    t2s = np.sort(rng.choice(n, m2, replace=False))
+    t0 = time.perf_counter()
+    orc.evaluate(w, mode="tree", targets=t2s)
+    T2 = time.perf_counter() - t0
+    if T2 - T1 < budget_s / 3.0 and m2 < n // 2:       # the first guess was too small: one larger sample
+        m2 = int(min(n // 2, m2 * budget_s / max(T2 - T1, 1e-3)))
+        t2s = np.sort(rng.choice(n, m2, replace=False))
+        t0 = time.perf_counter()
+        orc.evaluate(w, mode="tree", targets=t2s)
+        T2 = time.perf_counter() - t0
+    per = max((T2 - T1) / (m2 - m1), 1e-12)
+    fixed = max(T1 - per * m1, 0.0)
+    return fixed + per * n, (f"rates of {m2} random target particles of the full {n}-particle workload "
+                             f"({T2:.1f} s) and of {m1} ({T1:.1f} s); tree, order and pre-pass over all "
+                             f"particles both times; T(N) = {fixed:.2f} s + N * {per * 1e6:.2f} us")
+
+
+def host_cores():
+    v = os.environ.get("OMP_NUM_THREADS")
+    return int(v) if v else (os.cpu_count() or 1)
+
+
+def config_of_workload(w, args, extra=None):
+    c = {"workload": w.name, "n_particles": w.n, "dim": w.dim, "rhs_evaluations_per_step": 2, "dt": w.dt,
+         "flags": int(w.flags), "scale": args.scale}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def run_reference(args, rank, world):
+    """--impl reference: there is no upstream code (the reference is PAPER.md); the reference arm
+    is the CPU oracle, timed as it stands on the host cores, each step a bounded sample."""
+    if rank != 0:
+        return None
+    w = sph_inputs.make(args.workload, scale=args.scale)
+    per_step = []
+    sample = ""
+    for k in range(args.warmup + args.steps):
+        t_eval, sample = oracle_time(w, budget_s=6.0)
+        if k >= args.warmup:
+            per_step.append(2.0 * t_eval)            # a step is two evaluations
+        if sum(per_step) > 150.0:
+            break
+    T = float(np.mean(per_step))
+    value = 2.0 * w.n / T
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": len(per_step), "warmup": args.warmup, "ms_per_step": T * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_of_workload(w, args),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    return line
+
+
+def aggregate(ms_local, n_local, world, reduce_max, reduce_sum):
+    """Whole-job value from per-rank numbers: units all ranks processed / max over ranks of the time."""
+    ms = reduce_max(ms_local)
+    total = reduce_sum(n_local)
+    return ms, total
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(sph_inputs.CONFIGS))
+    ap.add_argument("--scale", type=float, default=1.0, help="< 1: smaller instance of the same workload (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+
+    if args.impl == "reference":
+        line = run_reference(args, rank, world)
+        if line is not None:
+            print(json.dumps(line), flush=True)
+        return 0
+
+    import torch
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.distributed.init_process_group("nccl")
+
+    r = run_ours(args, rank, world)
+    w = r["w"]
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", rank)))
+
+    def reduce(x, op):
+        if world == 1:
+            return float(x)
+        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=op)
+        return float(t.item())
+
+    rmax = lambda x: reduce(x, torch.distributed.ReduceOp.MAX if world > 1 else None)
+    rsum = lambda x: reduce(x, torch.distributed.ReduceOp.SUM if world > 1 else None)
+    ms_dev, n_total = aggregate(r["ms_dev"], w.n, world, rmax, rsum)
+    ms_e2e, _ = aggregate(r["ms_e2e"], w.n, world, rmax, rsum)
+    launches = int(rsum(r["launches"]))
+    if rank != 0:
+        torch.distributed.destroy_process_group()
+        return 0
+
+    evals = 2 * args.steps
+    value = n_total * evals / (ms_dev * 1e-3)
+    e2e_value = n_total * 2 / (ms_e2e * 1e-3)
+    hbm_peak, hbm_src = _peaks()
+
+    # per-stage table and rooflines (rank 0's replica)
+    tot_ms = sum(v[0] for v in r["stages"].values()) or 1.0
+    stages, roofs = {}, {}
+    for name, (ms, ln) in r["stages"].items():
+        if ln == 0:
+            continue
+        bound, unit, amount = stage_work(name, w, r["counters"], evals)
+        calls = evals
+        avg_ms = ms / calls
+        ach = amount / (avg_ms * 1e-3) * (1e-12 if bound == "alu" else 1e-9)
+        peak = r["fp64_peak"] if bound == "alu" else hbm_peak
+        stages[name] = {"ms_per_eval": round(avg_ms, 4), "share": round(ms / tot_ms, 4), "launches_per_eval": ln / calls}
+        roofs[name] = {"bound": bound, "achieved": round(ach, 3), "peak": round(peak, 2), "unit": unit,
+                       "frac": round(ach / peak, 4)}
+    top = max(stages, key=lambda k: stages[k]["share"])
+    roofline = dict(roofs[top])
+    roofline.update({"kernel": top, "traffic": TRAFFIC_NCU.get((args.workload, top)),
+                     "peak_source": ("FP64 FMA micro-benchmark measured in this run (sph_measure_fp64_peak); nominal "
+                                     "148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s") if roofline["bound"] == "alu"
+                     else hbm_src})
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_dev / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_of_workload(w, args, {
+                "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                "l2": "L2 flushed (252 MB write) between timed steps" if r["l2_flush"]
+                      else "working set larger than L2 (%.1f GB workspace)" % (r["ws_bytes"] / 1e9),
+                "particle_steps_per_s": n_total * args.steps / (ms_dev * 1e-3),
+                "counters_last_eval": r["counters"]}),
+            "clocks": r["clocks"],
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(r["h2d"]),
+                    "d2h_bytes_per_step": int(r["d2h"]), "ms_per_step": ms_e2e},
+            "gpu_launches": launches,
+            "roofline": roofline, "stages": stages, "rooflines_all": roofs}
+    if world == 1 and not args.no_cpu_baseline:
+        t_eval, sample = oracle_time(w)
+        line["cpu_baseline"] = {"value": w.n / t_eval, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
+                                "sample": sample}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures under profiles/ (filled in per round; None = not captured yet).
+TRAFFIC_NCU = {}
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -162,8 +162,42 @@ int sph_get_tree(sph_ctx *ctx, int32_t *level, uint64_t *prefix, int32_t *lo, in
 /* CSR partner lists in ORIGINAL indices, ascending per particle. off[n+1]; idx[cap]. Returns
  * SPH_ERR_ARG if cap is too small (off is still filled, so off[n] tells the needed size). */
 int sph_get_neighbours(sph_ctx *ctx, int64_t *off, int32_t *idx, int64_t cap);
-/* Per-call kernel time accounting: number of kernels launched by this context so far. */
+/* Number of kernels launched by this context so far. */
 int64_t sph_launch_count(sph_ctx *ctx);
+
+/* ---- measurement ---- */
+/* Stages of one right-hand-side evaluation, in the sub-step order of PAPER.md:693. */
+enum {
+    SPH_T_KEYS = 0,     /* A1  bounding cube (eq. 67) + Morton keys                         */
+    SPH_T_SORT,         /* A2  radix sort of (key, index)                                  */
+    SPH_T_REORDER,      /* A2  SoA gather into Morton order                                */
+    SPH_T_TREE,         /* A3  octree topology (node discovery, node sort, child tables)   */
+    SPH_T_MOMENTS,      /* A4  pseudo-particles: mass, centre of mass, boxes, hmax         */
+    SPH_T_NEIGHBOURS,   /* A5  interaction-partner search (+ eq. 73)                       */
+    SPH_T_DENSITY,      /* A6  density sum, eq. 28                                         */
+    SPH_T_PREPASS,      /* A7  EoS, limiter, damaged stress                                */
+    SPH_T_PAIRS,        /* A8-A10 pair sums + correction tensor + dS/dt + damage epilogue  */
+    SPH_T_GRAVITY,      /* A11 Barnes-Hut walk                                             */
+    SPH_T_UPDATE,       /* A12 predictor / corrector update                                */
+    SPH_T_COUNT
+};
+/* on != 0: bracket every stage with a pair of CUDA events on the context's stream (two event
+ * records per stage, no synchronisation); on == 0: stop and drop pending records. */
+int sph_timing_enable(sph_ctx *ctx, int on);
+/* Synchronises the stream and ADDS the device time [ms] and the number of kernel launches of every
+ * stage bracket recorded since the last read into ms[SPH_T_COUNT] / launches[SPH_T_COUNT] (HOST). */
+int sph_timing_read(sph_ctx *ctx, double *ms, int64_t *launches);
+const char *sph_timing_name(int stage);
+/* Work counters of the LAST evaluation (HOST out[4]; synchronises): internal nodes; sum over
+ * particles of the partner count; sum over particles of gravity interactions (accepted pseudo-
+ * particles + directly summed particles, eq. 51); sum over particles of opening tests (eq. 50). */
+int sph_get_counters(sph_ctx *ctx, int64_t *out);
+/* Dependency-free FP64 FMA throughput of the device [TFLOP/s] (the ALU roofline denominator;
+ * MEASURED_PEAKS.json has no FP64 figure). stream: cudaStream_t. Synchronises. */
+int sph_measure_fp64_peak(void *cuda_stream, double *tflops);
+/* Streaming FP64 copy bandwidth [GB/s, read + write bytes] over `bytes` of the workspace-free
+ * scratch the caller provides (DEVICE src, dst). Synchronises. */
+int sph_measure_copy_bw(void *cuda_stream, const double *src, double *dst, size_t bytes, double *gbs);
 
 const char *sph_last_error(sph_ctx *ctx);
 const char *sph_version(void);

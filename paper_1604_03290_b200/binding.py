@@ -22,7 +22,9 @@ SPH_F_SOLID, SPH_F_PLASTIC, SPH_F_DAMAGE, SPH_F_GRAVITY, SPH_F_VARIABLE_H, SPH_F
 EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sph_build_tree",
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
-           "sph_launch_count", "sph_last_error", "sph_version"]
+           "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
+           "sph_timing_name", "sph_get_counters", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+SPH_T_COUNT = 11
 
 _vp = C.c_void_p
 
@@ -93,6 +95,13 @@ def load_library():
     L.sph_last_error.restype = C.c_char_p
     L.sph_last_error.argtypes = [_vp]
     L.sph_version.restype = C.c_char_p
+    L.sph_timing_enable.argtypes = [_vp, C.c_int]
+    L.sph_timing_read.argtypes = [_vp, _vp, _vp]
+    L.sph_timing_name.restype = C.c_char_p
+    L.sph_timing_name.argtypes = [C.c_int]
+    L.sph_get_counters.argtypes = [_vp, _vp]
+    L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
+    L.sph_measure_copy_bw.argtypes = [_vp, _vp, _vp, C.c_size_t, C.POINTER(C.c_double)]
     _lib = L
     return L
 
@@ -282,6 +291,21 @@ class Context:
     def launch_count(self):
         return int(load_library().sph_launch_count(self.handle))
 
+    def timing_enable(self, on=True):
+        self._check(load_library().sph_timing_enable(self.handle, int(bool(on))))
+
+    def timing_read(self):
+        """dict stage name -> (device ms, kernel launches) accumulated since the previous read."""
+        L = load_library()
+        ms, ln = np.zeros(SPH_T_COUNT), np.zeros(SPH_T_COUNT, np.int64)
+        self._check(L.sph_timing_read(self.handle, ms.ctypes.data, ln.ctypes.data))
+        return {L.sph_timing_name(k).decode(): (float(ms[k]), int(ln[k])) for k in range(SPH_T_COUNT)}
+
+    def get_counters(self):
+        out = np.zeros(4, np.int64)
+        self._check(load_library().sph_get_counters(self.handle, out.ctypes.data))
+        return dict(n_nodes=int(out[0]), n_pairs=int(out[1]), n_inter=int(out[2]), n_visit=int(out[3]))
+
 
 # ---- module-level functions with the names of the C ABI ----
 def sph_version():
@@ -334,3 +358,27 @@ def sph_download(ctx, fields=STATE_FIELDS + RATE_FIELDS, device=False, out=None)
 
 def sph_sync(ctx):
     ctx.sync()
+
+
+def sph_measure_fp64_peak(stream=None):
+    """Dependency-free FP64 FMA throughput of the current device, TFLOP/s."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    v = C.c_double()
+    rc = load_library().sph_measure_fp64_peak(_vp(st.cuda_stream), C.byref(v))
+    if rc != SPH_OK:
+        raise SphError(rc, "sph_measure_fp64_peak")
+    return v.value
+
+
+def sph_measure_copy_bw(nbytes=1 << 30, stream=None):
+    """Streaming FP64 copy bandwidth (read + write bytes), GB/s."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    a = torch.zeros(nbytes // 8, dtype=torch.float64, device="cuda")
+    b = torch.empty_like(a)
+    v = C.c_double()
+    rc = load_library().sph_measure_copy_bw(_vp(st.cuda_stream), _vp(a.data_ptr()), _vp(b.data_ptr()), nbytes, C.byref(v))
+    if rc != SPH_OK:
+        raise SphError(rc, "sph_measure_copy_bw")
+    return v.value

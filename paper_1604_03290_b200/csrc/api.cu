@@ -116,6 +116,39 @@ struct sph_ctx_ext {
     Mats *mats_dev;
 };
 
+// ------------------------------------------------------------------------------------------------
+// stage timing: event pairs on the context's stream, resolved by sph_timing_read
+// ------------------------------------------------------------------------------------------------
+struct SphTiming {
+    struct Rec { int stage; cudaEvent_t e0, e1; i64 l0, l1; };
+    std::vector<Rec> pending;
+    std::vector<cudaEvent_t> pool;
+    cudaEvent_t get() {
+        if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+        cudaEvent_t e; cudaEventCreate(&e); return e;
+    }
+    ~SphTiming() {
+        for (auto &r : pending) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+        for (auto e : pool) cudaEventDestroy(e);
+    }
+};
+
+void sph_timing_begin(sph_ctx *ctx, int stage) {
+    SphTiming *t = ctx->timing;
+    SphTiming::Rec r{stage, t->get(), t->get(), ctx->launches, 0};
+    cudaEventRecord(r.e0, ctx->stream);
+    t->pending.push_back(r);
+}
+void sph_timing_end(sph_ctx *ctx, int stage) {
+    SphTiming *t = ctx->timing;
+    for (size_t k = t->pending.size(); k-- > 0;)
+        if (t->pending[k].stage == stage && t->pending[k].l1 == 0) {
+            cudaEventRecord(t->pending[k].e1, ctx->stream);
+            t->pending[k].l1 = ctx->launches + 1;   // +1 so that 0 means "open"
+            return;
+        }
+}
+
 static inline sph_ctx_ext *ext(sph_ctx *c) { return (sph_ctx_ext *)c; }
 const sph_material *sph_dev_mats(sph_ctx *ctx) { return ext(ctx)->mats_dev->m; }
 
@@ -247,7 +280,49 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
 void sph_destroy(sph_ctx *ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    delete ctx->timing;
     delete ext(ctx);
+}
+
+int sph_timing_enable(sph_ctx *ctx, int on) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (on && !ctx->timing) ctx->timing = new (std::nothrow) SphTiming();
+    if (!on && ctx->timing) { cudaStreamSynchronize(ctx->stream); delete ctx->timing; ctx->timing = nullptr; }
+    return SPH_OK;
+}
+
+int sph_timing_read(sph_ctx *ctx, double *ms, int64_t *launches) {
+    if (!ctx || !ms || !launches) return SPH_ERR_ARG;
+    if (!ctx->timing) return fail(ctx, SPH_ERR_STATE, "sph_timing_read before sph_timing_enable");
+    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_timing_read");
+    SphTiming *t = ctx->timing;
+    for (auto &r : t->pending) {
+        if (r.l1 != 0) {
+            float e = 0.f;
+            if (cudaEventElapsedTime(&e, r.e0, r.e1) == cudaSuccess && r.stage >= 0 && r.stage < SPH_T_COUNT) {
+                ms[r.stage] += (double)e;
+                launches[r.stage] += (r.l1 - 1) - r.l0;
+            }
+        }
+        t->pool.push_back(r.e0); t->pool.push_back(r.e1);
+    }
+    t->pending.clear();
+    return check_cuda(ctx, "sph_timing_read");
+}
+
+const char *sph_timing_name(int stage) {
+    static const char *names[SPH_T_COUNT] = {"keys", "sort", "reorder", "tree", "moments", "neighbours",
+                                             "density", "prepass", "pairs", "gravity", "update"};
+    return (stage >= 0 && stage < SPH_T_COUNT) ? names[stage] : "?";
+}
+
+int sph_get_counters(sph_ctx *ctx, int64_t *out) {
+    if (!ctx || !out) return SPH_ERR_ARG;
+    DevStatus st;
+    cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    out[0] = st.n_nodes; out[1] = (int64_t)st.n_pairs; out[2] = (int64_t)st.n_inter; out[3] = (int64_t)st.n_visit;
+    return check_cuda(ctx, "sph_get_counters");
 }
 
 int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
@@ -316,13 +391,22 @@ int sph_step(sph_ctx *ctx, double dt) {
     Dev &d = ctx->d;
     const size_t n = (size_t)d.n;
     int rc;
-    cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    {
+        StageTimer tm(ctx, SPH_T_UPDATE);
+        cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    }
     if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
-    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), 0.5 * dt, 0);   // eq. 52
-    ctx->launches += 1;
+    {
+        StageTimer tm(ctx, SPH_T_UPDATE);
+        k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), 0.5 * dt, 0);   // eq. 52
+        ctx->launches += 1;
+    }
     if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
-    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, 1);         // eq. 53
-    ctx->launches += 1;
+    {
+        StageTimer tm(ctx, SPH_T_UPDATE);
+        k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, 1);         // eq. 53
+        ctx->launches += 1;
+    }
     ctx->have_tree = ctx->have_lists = 0;   // the state moved on; the rates stay readable
     return check_cuda(ctx, "sph_step");
 }

@@ -167,9 +167,12 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
         if (valid) d.nb_cnt[i] = min(cnt, d.cap);
         int mx = cnt;
         for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
+        int tot = valid ? min(cnt, d.cap) : 0;
+        for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(FULL, tot, o);
         if (lane == 0) {
             if (mx > d.cap) atomicExch(&d.status->err_nb_overflow, 1);
             atomicMax(&d.status->nb_max, mx);
+            atomicAdd(&d.status->n_pairs, (u64)tot);
         }
     }
 }
@@ -224,6 +227,7 @@ void sph_stage_writeback_h(sph_ctx *ctx) {
 
 void sph_stage_neigh(sph_ctx *ctx) {
     Dev &d = ctx->d;
+    StageTimer tm(ctx, SPH_T_NEIGHBOURS);
     const bool varh = (d.flags & SPH_F_VARIABLE_H) != 0;
     if (varh && ctx->cfg.h_iters > 0) {
         for (int it = 0; it < ctx->cfg.h_iters; ++it) {

@@ -222,15 +222,22 @@ void sph_stage_order(sph_ctx *ctx) {
     Dev &d = ctx->d;
     const int n = d.n;
     int nb = min(sph_ceil_div(n, 256), 1024);
-    k_bbox_partial<<<nb, 256, 0, ctx->stream>>>(d, nb);
-    k_bbox_final<<<1, 32, 0, ctx->stream>>>(d, nb);
-    k_keys<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
-    ctx->launches += 3;
+    {
+        StageTimer tm(ctx, SPH_T_KEYS);
+        k_bbox_partial<<<nb, 256, 0, ctx->stream>>>(d, nb);
+        k_bbox_final<<<1, 32, 0, ctx->stream>>>(d, nb);
+        k_keys<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
+        ctx->launches += 3;
+    }
     int cur = 0;
-    sph_radix_sort(ctx, d.key, d.idx, n, nullptr, d.D * d.L, &cur);
+    {
+        StageTimer tm(ctx, SPH_T_SORT);
+        sph_radix_sort(ctx, d.key, d.idx, n, nullptr, d.D * d.L, &cur);
+    }
     d.keys = d.key[cur];
     d.perm = d.idx[cur];
     ctx->sort_cur = cur;
+    StageTimer tm(ctx, SPH_T_REORDER);
     k_gather<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
     ctx->launches += 1;
 }

@@ -324,11 +324,17 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
     const bool varh = (d.flags & SPH_F_VARIABLE_H) != 0, solid = (d.flags & SPH_F_SOLID) != 0;
     const int gb = sph_ceil_div((i64)sph_ceil_div(n, 32) * 32, 128);
     if (d.flags & SPH_F_DENSITY_SUM) {
+        StageTimer tm(ctx, SPH_T_DENSITY);
         if (varh) k_density<D, true><<<gb, 128, 0, ctx->stream>>>(d);
         else k_density<D, false><<<gb, 128, 0, ctx->stream>>>(d);
         ctx->launches += 1;
     }
-    k_prepass<D><<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d, mats);
+    {
+        StageTimer tm(ctx, SPH_T_PREPASS);
+        k_prepass<D><<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d, mats);
+        ctx->launches += 1;
+    }
+    StageTimer tm(ctx, SPH_T_PAIRS);
     if (solid) {
         if (varh) k_pairs<D, true, true><<<gb, 128, 0, ctx->stream>>>(d, mats);
         else k_pairs<D, true, false><<<gb, 128, 0, ctx->stream>>>(d, mats);
@@ -336,7 +342,7 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
         if (varh) k_pairs<D, false, true><<<gb, 128, 0, ctx->stream>>>(d, mats);
         else k_pairs<D, false, false><<<gb, 128, 0, ctx->stream>>>(d, mats);
     }
-    ctx->launches += 2;
+    ctx->launches += 1;
 }
 
 const sph_material *sph_dev_mats(sph_ctx *ctx);

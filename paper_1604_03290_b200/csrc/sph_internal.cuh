@@ -10,6 +10,7 @@
 typedef unsigned long long u64;
 typedef long long i64;
 
+
 #define SPH_MAX_MAT 16
 #define SPH_WARP 32
 
@@ -19,7 +20,11 @@ struct DevStatus {
     int err_nb_overflow;
     int err_stack;
     int nb_max;         // largest partner count seen
-    int pad[4];
+    // work counters of the last evaluation (algorithmic units for the roofline)
+    u64 n_pairs;        // sum over particles of |N(a)|               (A5)
+    u64 n_inter;        // accepted pseudo-particles + direct particles, per particle, summed (A11)
+    u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
+    u64 pad;
 };
 
 // Root cube of the last build (device).
@@ -81,6 +86,8 @@ struct Dev {
     int *stage_i;               // n ints
 };
 
+struct SphTiming;   // api.cu: CUDA-event pairs around the stages (sph_timing_*)
+
 struct sph_ctx {
     sph_config cfg;
     Dev d;
@@ -91,7 +98,17 @@ struct sph_ctx {
     int have_state, have_tree, have_lists, have_rates;
     i64 launches;
     int sort_cur;
+    SphTiming *timing;          // NULL unless sph_timing_enable(ctx, 1)
     char err[512];
+};
+
+// RAII bracket of one stage: two event records on ctx->stream when timing is enabled, nothing otherwise.
+void sph_timing_begin(sph_ctx *ctx, int stage);
+void sph_timing_end(sph_ctx *ctx, int stage);
+struct StageTimer {
+    sph_ctx *c; int stage;
+    StageTimer(sph_ctx *ctx, int st) : c(ctx), stage(st) { if (c->timing) sph_timing_begin(c, stage); }
+    ~StageTimer() { if (c->timing) sph_timing_end(c, stage); }
 };
 
 #define SPH_LAUNCH(ctx) ((ctx)->launches++)

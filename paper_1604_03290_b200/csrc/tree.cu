@@ -153,11 +153,13 @@ __global__ void k_moments(Dev d, int level) {
 
 __global__ void k_zero_status(Dev d) {
     d.status->n_nodes = 0;
+    d.status->n_pairs = 0; d.status->n_inter = 0; d.status->n_visit = 0;
 }
 
 void sph_stage_tree(sph_ctx *ctx) {
     Dev &d = ctx->d;
     const int n = d.n;
+    StageTimer *tt = new StageTimer(ctx, SPH_T_TREE);
     k_zero_status<<<1, 1, 0, ctx->stream>>>(d);
     k_find_nodes<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
     ctx->launches += 2;
@@ -167,6 +169,8 @@ void sph_stage_tree(sph_ctx *ctx) {
     sph_radix_sort(ctx, d.nkey, d.nhi, n, &d.status->n_nodes, bits, &cur);
     k_fill_nodes<<<sph_ceil_div(n, 128), 128, 0, ctx->stream>>>(d, d.nkey[cur], d.nhi[cur]);
     ctx->launches += 1;
+    delete tt;
+    StageTimer tm(ctx, SPH_T_MOMENTS);
     for (int lvl = d.L - 1; lvl >= 0; --lvl) {
         k_moments<<<sph_ceil_div(n, 128), 128, 0, ctx->stream>>>(d, lvl);
         ctx->launches += 1;
