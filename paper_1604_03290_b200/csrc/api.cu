@@ -81,6 +81,10 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.nmass = b.take<double>(n);
     for (int a = 0; a < 3; ++a) { z.ncom[a] = b.take<double>(n); z.nbmin[a] = b.take<double>(n); z.nbmax[a] = b.take<double>(n); }
     z.nhmax = b.take<double>(n); z.ns2 = b.take<double>(n);
+    z.items = b.take<SearchItem>(2 * n + 2);
+    z.witems = b.take<WalkItem>((c->flags & SPH_F_GRAVITY) ? 2 * n + 2 : 1);
+    z.bmark = b.take<u64>(n + 1); z.bscan = b.take<u64>(n + 1);
+    z.scan_tmp = b.take<u64>(sph_scan_scratch_elems((i64)n + 1) + 2);
     z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);
     z.nb_cnt = b.take<int>(n); z.own_cnt = b.take<int>(n);
     z.p = b.take<double>(n); z.cs = b.take<double>(n); z.vol = b.take<double>(n);

@@ -2,27 +2,129 @@
 //
 // The paper walks the tree once per particle, one thread each, descending while the particle lies
 // within s/2 + h of a cell (eq. 69) and testing "distance < smoothing length" at the leaves.
-// Here one WARP owns 32 particles that are consecutive in Morton order.  The warp walks the tree
-// once for the group's bounding box grown by the reach (lanes test 2^D children of several nodes
-// in parallel against the nodes' tight bounding boxes and hmax), collects candidate particles in
-// shared memory, stages 32 candidates at a time (coalesced loads), and every lane applies the
-// exact membership test of the paper to its own particle:
-//     r^2 = (dx*dx + dy*dy) + dz*dz  <  H*H,   H = h_a, or (h_a + h_b)/2 with variable h (eq. 72)
-// with every operation rounded separately, so the sets equal the oracle's bit for bit.
+// Here one WARP owns 32 particles that are consecutive in Morton order and walks ONE stream for
+// all of them, but every lane prunes for its own particle:
+//
+//   * The search stream (built by sph_build_search_items below) holds, in depth-first pre-order,
+//     the octree cells with more than SPH_BUCKET particles and BUCKETS of <= SPH_BUCKET particles
+//     that are consecutive in Morton order (runs of small sibling cells / leaves).  Every record
+//     carries the tight bounding box and the largest h of the particles below it.
+//   * Every lane keeps the index of the next record IT has to look at: a cell whose box is out
+//     of the lane's reach is skipped (next = skip index), otherwise entered (next = cur + 1).
+//     The warp visits min over lanes(next) (one redux.sync), so the records a warp touches are
+//     the union of 32 single-particle walks -- bounded even where the Morton curve jumps and a
+//     group's bounding box spans half a body (profiles/r1a_c5_first_path.md: that tail cost 96 %).
+//   * A bucket within reach of any lane is staged through shared memory with one coalesced load
+//     per coordinate, and every lane applies the exact membership test of the paper to its own
+//     particle:   r^2 = (dx*dx + dy*dy) + dz*dz  <  H*H,   H = h_a, or (h_a + h_b)/2 with variable
+//     h (eq. 72), every operation rounded separately, so the sets equal the oracle's bit for bit.
 // Lists are written group-transposed, nb[(group*cap + k)*32 + lane], so that the pair-sum kernel
-// reads them fully coalesced.
+// reads them fully coalesced; within a list partners come in ascending Morton order.
 #include "sph_internal.cuh"
 
-#define NB_WARPS 4
-#define NB_STACK 1024
+#define NB_WARPS 8
 
+// ------------------------------------------------------------------------------------------
+// search stream layout
+// ------------------------------------------------------------------------------------------
+// bmark[i]: low word 1 = a bucket starts at sorted particle i; high word = number of big cells
+// whose range starts at i.
+__global__ void k_mark_buckets(Dev d) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nn = d.status->n_nodes, n = d.n;
+    if (nn == 0) {   // n == 1 or all keys equal: plain runs of SPH_BUCKET
+        if (t < n && (t % SPH_BUCKET) == 0) d.bmark[t] = 1ull;
+        return;
+    }
+    if (t >= nn) return;
+    const int NC = 1 << d.D;
+    const int lo = d.nlo[t], hi = d.nhi_s[t];
+    if (hi - lo <= SPH_BUCKET) {
+        if (t == 0) d.bmark[0] = 1ull;          // the whole set is one bucket
+        return;
+    }
+    atomicAdd(&d.bmark[lo], 1ull << 32);
+    const int *cl = d.child_lo + (size_t)t * (NC + 1);
+    const int *ch = d.child + (size_t)t * NC;
+    bool open = false;
+    int run = 0;
+    for (int c = 0; c < NC; ++c) {
+        const int r0 = cl[c], r1 = cl[c + 1], sz = r1 - r0;
+        if (sz == 0) continue;
+        if (sz > SPH_BUCKET) {
+            // a big child cell lays itself out; a leaf of > SPH_BUCKET coincident particles is cut into runs
+            if (ch[c] == -2) for (int p = r0; p < r1; p += SPH_BUCKET) atomicAdd(&d.bmark[p], 1ull);
+            open = false;
+            continue;
+        }
+        if (open && run + sz <= SPH_BUCKET) run += sz;           // merge small siblings
+        else { atomicAdd(&d.bmark[r0], 1ull); open = true; run = sz; }
+    }
+}
+
+__global__ void k_emit_items(Dev d) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n = d.n, nn = d.status->n_nodes;
+    const int D = d.D;
+    if (t == 0) {
+        const u64 tot = d.bscan[n];
+        d.status->n_items = (int)(tot & 0xffffffffu) + (int)(tot >> 32);
+    }
+    if (t < n && (d.bmark[t] & 1ull)) {          // bucket starting at t
+        const u64 sc = d.bscan[t];
+        const int pos = (int)(sc & 0xffffffffu) + (int)(sc >> 32) + (int)(d.bmark[t] >> 32);
+        int e = t + 1;
+        while (e < n && !(d.bmark[e] & 1ull)) ++e;
+        SearchItem it;
+        double hm = 0.0;
+        for (int a = 0; a < 3; ++a) { it.bmin[a] = INFINITY; it.bmax[a] = -INFINITY; }
+        for (int p = t; p < e; ++p) {
+            for (int a = 0; a < D; ++a) {
+                const double x = d.sx[a][p];
+                it.bmin[a] = fmin(it.bmin[a], x); it.bmax[a] = fmax(it.bmax[a], x);
+            }
+            hm = fmax(hm, d.sh[p]);
+        }
+        for (int a = D; a < 3; ++a) { it.bmin[a] = 0.0; it.bmax[a] = 0.0; }
+        it.hmax = hm; it.skip = -(e - t); it.lo = t;
+        d.items[pos] = it;
+    }
+    if (t < nn) {
+        const int lo = d.nlo[t], hi = d.nhi_s[t];
+        if (hi - lo > SPH_BUCKET) {              // big cell
+            int k = 0;
+            while (t - 1 - k >= 0 && d.nlo[t - 1 - k] == lo) ++k;     // ancestors sharing lo precede it
+            const u64 sl = d.bscan[lo], sh_ = d.bscan[hi];
+            SearchItem it;
+            for (int a = 0; a < 3; ++a) { it.bmin[a] = d.nbmin[a][t]; it.bmax[a] = d.nbmax[a][t]; }
+            it.hmax = d.nhmax[t];
+            it.skip = (int)(sh_ & 0xffffffffu) + (int)(sh_ >> 32);
+            it.lo = lo;
+            d.items[(int)(sl & 0xffffffffu) + (int)(sl >> 32) + k] = it;
+        }
+    }
+}
+
+static void emit_items(sph_ctx *ctx) {
+    k_emit_items<<<sph_ceil_div(ctx->d.n, 128), 128, 0, ctx->stream>>>(ctx->d);
+    ctx->launches += 1;
+}
+
+void sph_build_search_items(sph_ctx *ctx) {
+    Dev &d = ctx->d;
+    cudaMemsetAsync(d.bmark, 0, ((size_t)d.n + 1) * sizeof(u64), ctx->stream);
+    k_mark_buckets<<<sph_ceil_div(d.n, 128), 128, 0, ctx->stream>>>(d);
+    ctx->launches += 1;
+    sph_scan_u64(ctx, d.bmark, d.bscan, (i64)d.n + 1, d.scan_tmp);
+    emit_items(ctx);
+}
+
+// ------------------------------------------------------------------------------------------
+// the walk
+// ------------------------------------------------------------------------------------------
 template <int D, bool VARH, bool COUNT_ONLY>
 __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
-    constexpr int NC = 1 << D;
-    __shared__ int s_stack[NB_WARPS][NB_STACK];
-    __shared__ int s_cand[NB_WARPS][64];
     __shared__ double s_c[NB_WARPS][4][32];
-    __shared__ int s_ci[NB_WARPS][32];
 
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = blockIdx.x * NB_WARPS + w;
@@ -31,146 +133,76 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     const int i = g * 32 + lane;
     const bool valid = i < n;
     const int ii = valid ? i : n - 1;
-    const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
+    const unsigned FULL = 0xffffffffu;
 
     const double xi = d.sx[0][ii], yi = d.sx[1][ii], zi = (D == 3) ? d.sx[2][ii] : 0.0;
     const double Hi = d.sh[ii];
     const double Hi2 = __dmul_rn(Hi, Hi);
-    double gmin[3] = {xi, yi, zi}, gmax[3] = {xi, yi, zi}, Hg = Hi;
-    for (int o = 16; o > 0; o >>= 1) {
-        for (int a = 0; a < D; ++a) {
-            gmin[a] = fmin(gmin[a], __shfl_xor_sync(FULL, gmin[a], o));
-            gmax[a] = fmax(gmax[a], __shfl_xor_sync(FULL, gmax[a], o));
-        }
-        Hg = fmax(Hg, __shfl_xor_sync(FULL, Hg, o));
-    }
+    const double slack = 1.0 + 1e-9;            // the pruning test must never cut a true partner
 
-    int cnt = 0, own = 0, top = 0, ncand = 0;
-    int *stack = s_stack[w], *cand = s_cand[w];
+    int cnt = 0;
     int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
+    const int cap = d.cap;
+    const int nitems = d.status->n_items;
+    const SearchItem *__restrict__ items = d.items;
 
-    auto flush = [&](int take) {
-        const int cj = (lane < take) ? cand[lane] : -1;
-        if (cj >= 0) {
-            s_c[w][0][lane] = d.sx[0][cj];
-            s_c[w][1][lane] = d.sx[1][cj];
-            s_c[w][2][lane] = (D == 3) ? d.sx[2][cj] : 0.0;
-            s_c[w][3][lane] = d.sh[cj];
-            s_ci[w][lane] = cj;
-        }
-        __syncwarp();
-        for (int j = 0; j < take; ++j) {
-            const int b = s_ci[w][j];
-            const double dx = __dsub_rn(xi, s_c[w][0][j]);
-            const double dy = __dsub_rn(yi, s_c[w][1][j]);
-            const double dz = (D == 3) ? __dsub_rn(zi, s_c[w][2][j]) : 0.0;
-            const double r2 = sph_r2_exact(dx, dy, dz, D);
-            if (COUNT_ONLY) {
-                if (valid && b != i && r2 < Hi2) ++own;
-            } else {
-                double H2 = Hi2;
-                if (VARH) {
-                    const double Hab = __dmul_rn(0.5, __dadd_rn(Hi, s_c[w][3][j]));
-                    H2 = __dmul_rn(Hab, Hab);
+    int next = valid ? 0 : 0x7fffffff;
+    int cur = 0;
+    while (cur < nitems) {
+        const double2 *rec = reinterpret_cast<const double2 *>(items + cur);
+        const double2 q0 = __ldg(rec), q1 = __ldg(rec + 1), q2 = __ldg(rec + 2), q3 = __ldg(rec + 3);
+        const double4 b0 = make_double4(q0.x, q0.y, q1.x, q1.y);      // bmin xyz, bmax x
+        const double4 b1 = make_double4(q2.x, q2.y, q3.x, q3.y);      // bmax yz, hmax, (skip, lo)
+        const int skip = __double2loint(b1.w), lo = __double2hiint(b1.w);
+        const bool act = (next == cur);
+        const double reach = ((VARH && !COUNT_ONLY) ? 0.5 * (Hi + b1.z) : Hi) * slack;
+        bool ov = act && (b0.x - xi <= reach) && (xi - b0.w <= reach) && (b0.y - yi <= reach) && (yi - b1.x <= reach);
+        if (D == 3) ov = ov && (b0.z - zi <= reach) && (zi - b1.y <= reach);
+        if (skip >= 0) {
+            if (act) next = ov ? cur + 1 : skip;
+        } else {
+            if (act) next = cur + 1;
+            if (__any_sync(FULL, ov)) {
+                const int m = -skip;
+                if (lane < m) {
+                    const int p = lo + lane;
+                    s_c[w][0][lane] = d.sx[0][p];
+                    s_c[w][1][lane] = d.sx[1][p];
+                    if (D == 3) s_c[w][2][lane] = d.sx[2][p];
+                    if (VARH && !COUNT_ONLY) s_c[w][3][lane] = d.sh[p];
                 }
-                if (valid && b != i && r2 < H2) {
-                    if (cnt < d.cap) nbw[(size_t)cnt * 32] = b;
-                    ++cnt;
-                }
-            }
-        }
-        __syncwarp();
-        // keep what is left
-        const int rest = ncand - take;
-        int keep = (lane < rest) ? cand[take + lane] : 0;
-        __syncwarp();
-        if (lane < rest) cand[lane] = keep;
-        ncand = rest;
-        __syncwarp();
-    };
-
-    const int nn = d.status->n_nodes;
-    if (nn == 0) {
-        // no internal node (n == 1 or all keys equal): every particle is a candidate
-        for (int p0 = 0; p0 < n; p0 += 32) {
-            if (p0 + lane < n) cand[lane] = p0 + lane;
-            ncand = min(32, n - p0);
-            __syncwarp();
-            flush(ncand);
-        }
-    } else {
-        if (lane == 0) stack[0] = 0;
-        top = 1;
-        __syncwarp();
-        bool fail = false;
-        while (top > 0) {
-            const int npop = min(top, 32 / NC);
-            const int j = lane / NC, c = lane % NC;
-            const int node = (j < npop) ? stack[top - 1 - j] : -1;
-            __syncwarp();
-            top -= npop;
-            int push = -1, c0 = 0, c1 = 0;
-            if (node >= 0) {
-                const int code = d.child[(size_t)node * NC + c];
-                if (code >= 0) {
-                    double reach = (VARH && !COUNT_ONLY) ? 0.5 * (Hg + d.nhmax[code]) : Hg;
-                    reach *= (1.0 + 1e-9);
-                    bool ov = true;
-                    for (int a = 0; a < D; ++a)
-                        ov = ov && (__dsub_rn(d.nbmin[a][code], gmax[a]) <= reach) &&
-                             (__dsub_rn(gmin[a], d.nbmax[a][code]) <= reach);
-                    if (ov) push = code;
-                } else if (code == -2) {
-                    c0 = d.child_lo[(size_t)node * (NC + 1) + c];
-                    c1 = d.child_lo[(size_t)node * (NC + 1) + c + 1];
-                    if (c1 - c0 == 1) {
-                        double reach = (VARH && !COUNT_ONLY) ? 0.5 * (Hg + d.sh[c0]) : Hg;
-                        reach *= (1.0 + 1e-9);
-                        bool in = true;
-                        for (int a = 0; a < D; ++a) {
-                            const double xb = d.sx[a][c0];
-                            in = in && (__dsub_rn(xb, gmax[a]) <= reach) && (__dsub_rn(gmin[a], xb) <= reach);
-                        }
-                        if (!in) c1 = c0;
+                __syncwarp();
+                for (int j = 0; j < m; ++j) {
+                    const double dx = __dsub_rn(xi, s_c[w][0][j]);
+                    const double dy = __dsub_rn(yi, s_c[w][1][j]);
+                    const double dz = (D == 3) ? __dsub_rn(zi, s_c[w][2][j]) : 0.0;
+                    const double r2 = sph_r2_exact(dx, dy, dz, D);
+                    double H2 = Hi2;
+                    if (VARH && !COUNT_ONLY) {
+                        const double Hab = __dmul_rn(0.5, __dadd_rn(Hi, s_c[w][3][j]));
+                        H2 = __dmul_rn(Hab, Hab);
+                    }
+                    if (valid && (lo + j != i) && r2 < H2) {
+                        if (!COUNT_ONLY && cnt < cap) nbw[(size_t)cnt * 32] = lo + j;
+                        ++cnt;
                     }
                 }
-            }
-            const unsigned pm = __ballot_sync(FULL, push >= 0);
-            if (top + __popc(pm) > NB_STACK) { fail = true; break; }
-            if (push >= 0) stack[top + __popc(pm & lt)] = push;
-            top += __popc(pm);
-            const unsigned sm_ = __ballot_sync(FULL, c1 - c0 == 1);
-            if (c1 - c0 == 1) cand[ncand + __popc(sm_ & lt)] = c0;
-            ncand += __popc(sm_);
-            __syncwarp();
-            while (ncand >= 32) flush(32);
-            unsigned mm = __ballot_sync(FULL, c1 - c0 > 1);
-            while (mm) {   // leaves holding several particles with one key (degenerate, rare)
-                const int src = __ffs(mm) - 1;
-                mm &= mm - 1;
-                const int r0 = __shfl_sync(FULL, c0, src), r1 = __shfl_sync(FULL, c1, src);
-                for (int p = r0; p < r1; p += 32) {
-                    if (p + lane < r1) cand[ncand + lane] = p + lane;
-                    ncand += min(32, r1 - p);
-                    __syncwarp();
-                    while (ncand >= 32) flush(32);
-                }
+                __syncwarp();
             }
         }
-        if (fail && lane == 0) atomicExch(&d.status->err_stack, 1);
-        if (ncand > 0) flush(ncand);
+        cur = __reduce_min_sync(FULL, next);
     }
 
     if (COUNT_ONLY) {
-        if (valid) d.own_cnt[i] = own;
+        if (valid) d.own_cnt[i] = cnt;
     } else {
-        if (valid) d.nb_cnt[i] = min(cnt, d.cap);
+        if (valid) d.nb_cnt[i] = min(cnt, cap);
         int mx = cnt;
         for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
-        int tot = valid ? min(cnt, d.cap) : 0;
+        int tot = valid ? min(cnt, cap) : 0;
         for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(FULL, tot, o);
         if (lane == 0) {
-            if (mx > d.cap) atomicExch(&d.status->err_nb_overflow, 1);
+            if (mx > cap) atomicExch(&d.status->err_nb_overflow, 1);
             atomicMax(&d.status->nb_max, mx);
             atomicAdd(&d.status->n_pairs, (u64)tot);
         }
@@ -192,7 +224,7 @@ __global__ void k_writeback_h(Dev d) {
     d.h[d.perm[i]] = d.sh[i];
 }
 
-// hmax of every node must follow the new h: recompute the moments pass cheaply (hmax only)
+// hmax of every cell must follow the new h (hmax only; the boxes are unchanged)
 __global__ void k_hmax(Dev d, int level) {
     const int nd = blockIdx.x * blockDim.x + threadIdx.x;
     if (nd >= d.status->n_nodes) return;
@@ -229,6 +261,7 @@ void sph_stage_neigh(sph_ctx *ctx) {
     Dev &d = ctx->d;
     StageTimer tm(ctx, SPH_T_NEIGHBOURS);
     const bool varh = (d.flags & SPH_F_VARIABLE_H) != 0;
+    sph_build_search_items(ctx);
     if (varh && ctx->cfg.h_iters > 0) {
         for (int it = 0; it < ctx->cfg.h_iters; ++it) {
             if (d.D == 3) launch_neigh<3>(ctx, varh, true); else launch_neigh<2>(ctx, varh, true);
@@ -238,6 +271,7 @@ void sph_stage_neigh(sph_ctx *ctx) {
                 k_hmax<<<sph_ceil_div(d.n, 128), 128, 0, ctx->stream>>>(d, lvl);
                 ctx->launches += 1;
             }
+            emit_items(ctx);                 // refresh hmax of the records
         }
         sph_stage_writeback_h(ctx);
     }

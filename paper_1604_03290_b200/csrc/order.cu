@@ -117,24 +117,6 @@ __global__ void k_sort_hist(const u64 *__restrict__ kin, int n_host, const int *
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
-__global__ void k_sort_scan(unsigned *hist, int total) {   // one block of 1024 threads, exclusive scan
-    __shared__ unsigned part[1024];
-    int per = (total + 1023) / 1024;
-    int b = threadIdx.x * per, e = min(b + per, total);
-    unsigned s = 0;
-    for (int i = b; i < e; ++i) s += hist[i];
-    part[threadIdx.x] = s;
-    __syncthreads();
-    for (int o = 1; o < 1024; o <<= 1) {
-        unsigned v = (threadIdx.x >= o) ? part[threadIdx.x - o] : 0;
-        __syncthreads();
-        part[threadIdx.x] += v;
-        __syncthreads();
-    }
-    unsigned run = part[threadIdx.x] - s;
-    for (int i = b; i < e; ++i) { unsigned v = hist[i]; hist[i] = run; run += v; }
-}
-
 __global__ void __launch_bounds__(SORT_THREADS)
 k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__restrict__ kout,
                int *__restrict__ vout, int n_host, const int *n_dev, int shift,
@@ -188,10 +170,10 @@ void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const in
     int c = *cur;
     for (int shift = 0; shift < bits; shift += 8) {
         k_sort_hist<<<nblocks, 256, 0, ctx->stream>>>(key[c], n_host, n_dev, shift, ctx->d.hist, nblocks);
-        k_sort_scan<<<1, 1024, 0, ctx->stream>>>(ctx->d.hist, 256 * nblocks);
+        sph_scan_u32(ctx, ctx->d.hist, ctx->d.hist, (i64)256 * nblocks, (unsigned *)ctx->d.scan_tmp);
         k_sort_scatter<<<nblocks, SORT_THREADS, 0, ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host,
                                                                   n_dev, shift, ctx->d.hist, nblocks);
-        ctx->launches += 3;
+        ctx->launches += 2;
         c ^= 1;
     }
     *cur = c;

@@ -24,7 +24,8 @@ struct DevStatus {
     u64 n_pairs;        // sum over particles of |N(a)|               (A5)
     u64 n_inter;        // accepted pseudo-particles + direct particles, per particle, summed (A11)
     u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
-    u64 pad;
+    int n_items;        // records of the partner-search stream
+    int pad;
 };
 
 // Root cube of the last build (device).
@@ -33,6 +34,24 @@ struct DevRoot {
     double s0;
     double scale;       // 2^L / s0
     double pad[3];
+};
+
+// One record of the partner-search stream (neigh.cu): the octree cells that hold more than
+// SPH_BUCKET particles ("big" cells) and buckets of <= SPH_BUCKET Morton-consecutive particles, in
+// depth-first pre-order.  skip >= 0: big cell, index of the first record after its subtree;
+// skip < 0: bucket of -skip particles starting at sorted index lo.
+#define SPH_BUCKET 32
+struct __align__(16) SearchItem {
+    double bmin[3], bmax[3];    // tight bounding box of the particles below
+    double hmax;                // largest smoothing length below
+    int skip, lo;
+};
+
+// One record of the gravity stream (gravity.cu): internal cells and leaf particles in pre-order.
+struct __align__(16) WalkItem {
+    double cx, cy, cz, gm;      // centre of mass (or particle position), G * mass
+    double s2;                  // squared cell edge (eq. 68); -1 for a leaf particle
+    int skip, leaf;             // first record after the subtree
 };
 
 struct Mats {
@@ -72,6 +91,11 @@ struct Dev {
     int *child;                 // NC per node: >=0 node, -1 empty, -2 leaf
     int *child_lo;              // NC+1 per node
     double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
+    // ---- partner-search stream ----
+    SearchItem *items;          // up to 2n records
+    WalkItem *witems;           // n + n_nodes records
+    u64 *bmark, *bscan;         // n+1 each: low word bucket starts, high word big cells per lo; scan
+    u64 *scan_tmp;              // scratch of the prefix sums
     // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
     int *nb;
     int *nb_cnt;
@@ -120,6 +144,11 @@ static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 // (n_host) or, if n_dev != NULL, from device memory (kernels early-exit; grids sized for n_host).
 // Result ends in key[*cur], val[*cur].
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur);
+
+// ---- scan.cu ---- exclusive prefix sums (in == out allowed); scratch[ceil(n/2048)] = grand total
+void sph_scan_u32(sph_ctx *ctx, const unsigned *in, unsigned *out, i64 n, unsigned *scratch);
+void sph_scan_u64(sph_ctx *ctx, const u64 *in, u64 *out, i64 n, u64 *scratch);
+size_t sph_scan_scratch_elems(i64 n);
 
 // ---- per-stage entry points (each enqueues kernels on ctx->stream) ----
 void sph_stage_order(sph_ctx *ctx);     // A1 + A2
