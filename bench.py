@@ -307,6 +307,20 @@ def run_reference(args, rank, world):
     return line
 
 
+def make_reducers(world, device):
+    """(max, sum) over ranks of one float through torch.distributed (identity for world == 1)."""
+    if world == 1:
+        return float, float
+    import torch
+
+    def reduce(x, op):
+        t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+        torch.distributed.all_reduce(t, op=op)
+        return float(t.item())
+
+    return (lambda x: reduce(x, torch.distributed.ReduceOp.MAX)), (lambda x: reduce(x, torch.distributed.ReduceOp.SUM))
+
+
 def aggregate(ms_local, n_local, world, reduce_max, reduce_sum):
     """Whole-job value from per-rank numbers: units all ranks processed / max over ranks of the time."""
     ms = reduce_max(ms_local)
@@ -344,15 +358,7 @@ def main():
     w = r["w"]
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", rank)))
 
-    def reduce(x, op):
-        if world == 1:
-            return float(x)
-        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=op)
-        return float(t.item())
-
-    rmax = lambda x: reduce(x, torch.distributed.ReduceOp.MAX if world > 1 else None)
-    rsum = lambda x: reduce(x, torch.distributed.ReduceOp.SUM if world > 1 else None)
+    rmax, rsum = make_reducers(world, dev)
     ms_dev, n_total = aggregate(r["ms_dev"], w.n, world, rmax, rsum)
     ms_e2e, _ = aggregate(r["ms_e2e"], w.n, world, rmax, rsum)
     launches = int(rsum(r["launches"]))
