@@ -82,7 +82,12 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     for (int a = 0; a < 3; ++a) { z.ncom[a] = b.take<double>(n); z.nbmin[a] = b.take<double>(n); z.nbmax[a] = b.take<double>(n); }
     z.nhmax = b.take<double>(n); z.ns2 = b.take<double>(n);
     z.items = b.take<SearchItem>(2 * n + 2);
-    z.witems = b.take<WalkItem>((c->flags & SPH_F_GRAVITY) ? 2 * n + 2 : 1);
+    const size_t ngr = (c->flags & SPH_F_GRAVITY) ? 2 * n + 2 : 1;
+    z.grec = b.take<GravRec>(ngr);
+    z.gmeta = b.take<GravMeta>(ngr);
+    z.gcnt = b.take<unsigned>((c->flags & SPH_F_GRAVITY) ? n + 1 : 1);
+    z.gfirst = b.take<unsigned>((c->flags & SPH_F_GRAVITY) ? n + 1 : 1);
+    z.gthr = b.take<double>(32);
     z.bmark = b.take<u64>(n + 1); z.bscan = b.take<u64>(n + 1);
     z.scan_tmp = b.take<u64>(sph_scan_scratch_elems((i64)n + 1) + 2);
     z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);

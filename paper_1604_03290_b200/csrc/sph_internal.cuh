@@ -47,12 +47,19 @@ struct __align__(16) SearchItem {
     int skip, lo;
 };
 
-// One record of the gravity stream (gravity.cu): internal cells and leaf particles in pre-order.
-struct __align__(16) WalkItem {
-    double cx, cy, cz, gm;      // centre of mass (or particle position), G * mass
-    double s2;                  // squared cell edge (eq. 68); -1 for a leaf particle
-    int skip, leaf;             // first record after the subtree
+// Gravity records (gravity.cu): one per octree cell and per leaf, the children of a cell contiguous.
+// GravRec: centre of mass (or particle position) and G * mass.  GravMeta: first = index of the first
+// child record (cell), or first sorted particle (multi-particle leaf); info = count << 8 | kind,
+// kind (5 bits) = level of the cell (0..21), GR_LEAF1 = single particle, GR_LEAFN = several particles in one
+// leaf (equal keys at the deepest level).
+struct __align__(32) GravRec {
+    double x, y, z, gm;
 };
+struct __align__(8) GravMeta {
+    int first, info;
+};
+#define GR_LEAF1 30
+#define GR_LEAFN 31
 
 struct Mats {
     sph_material m[SPH_MAX_MAT];
@@ -93,7 +100,10 @@ struct Dev {
     double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
     // ---- partner-search stream ----
     SearchItem *items;          // up to 2n records
-    WalkItem *witems;           // n + n_nodes records
+    GravRec *grec;              // n + n_nodes records
+    GravMeta *gmeta;
+    unsigned *gcnt, *gfirst;    // per cell: number of child records, index of the first
+    double *gthr;               // 32 acceptance thresholds on r^2 (eq. 50), by record kind
     u64 *bmark, *bscan;         // n+1 each: low word bucket starts, high word big cells per lo; scan
     u64 *scan_tmp;              // scratch of the prefix sums
     // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
