@@ -92,8 +92,8 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.scan_tmp = b.take<u64>(sph_scan_scratch_elems((i64)n + 1) + 2);
     z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);
     z.nb_cnt = b.take<int>(n); z.own_cnt = b.take<int>(n);
-    z.p = b.take<double>(n); z.cs = b.take<double>(n); z.vol = b.take<double>(n);
-    for (int k = 0; k < 6; ++k) z.sr2[k] = b.take<double>(n);
+    z.p = b.take<double>(n); z.cs = b.take<double>(n);
+    z.prec = b.take<double>(n * PR_REC);
     z.drho = b.take<double>(n); z.du = b.take<double>(n); z.ddmg = b.take<double>(n); z.strain = b.take<double>(n);
     for (int a = 0; a < 3; ++a) { z.dv[a] = b.take<double>(n); z.ag[a] = b.take<double>(n); }
     for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(n);

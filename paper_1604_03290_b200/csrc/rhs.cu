@@ -75,10 +75,18 @@ __global__ void k_prepass(Dev d, const sph_material *mats) {
     for (int k = 0; k < 6; ++k) sg[k] = (1.0 - dd) * S[k];
     sg[0] -= phat; sg[3] -= phat;
     if (D == 3) sg[5] -= phat;
-    for (int k = 0; k < 6; ++k) d.sr2[k][i] = sg[k] * ir2;
     d.p[i] = p;
     d.cs[i] = cs;
-    d.vol[i] = d.sm[i] / rho;
+    // packed 128-byte record read by the pair kernel (one cache line per partner)
+    double2 *rec = reinterpret_cast<double2 *>(d.prec + (size_t)i * PR_REC);
+    rec[0] = make_double2(d.sx[0][i], d.sx[1][i]);
+    rec[1] = make_double2((D == 3) ? d.sx[2][i] : 0.0, d.sv[0][i]);
+    rec[2] = make_double2(d.sv[1][i], (D == 3) ? d.sv[2][i] : 0.0);
+    rec[3] = make_double2(rho, d.sm[i] / rho);
+    rec[4] = make_double2(cs, d.sh[i]);
+    rec[5] = make_double2(sg[0] * ir2, sg[1] * ir2);
+    rec[6] = make_double2(sg[2] * ir2, sg[3] * ir2);
+    rec[7] = make_double2(sg[4] * ir2, sg[5] * ir2);
 }
 
 template <int D> struct KNorm;
@@ -116,65 +124,152 @@ __global__ void __launch_bounds__(128) k_density(Dev d) {
     if (valid) { d.srho[i] = rho; d.rho[d.perm[i]] = rho; }
 }
 
-// largest eigenvalue of a symmetric DxD matrix, cyclic Jacobi
-template <int D>
-__device__ double max_eig_jacobi(double A[3][3]) {
-    for (int sweep = 0; sweep < 32; ++sweep) {
-        double off = 0.0;
-        for (int i = 0; i < D; ++i) for (int j = i + 1; j < D; ++j) off += A[i][j] * A[i][j];
-        if (off == 0.0) break;
-        for (int p = 0; p < D; ++p) for (int q = p + 1; q < D; ++q) {
-            if (A[p][q] == 0.0) continue;
-            const double th = (A[q][q] - A[p][p]) / (2.0 * A[p][q]);
-            const double t = ((th >= 0.0) ? 1.0 : -1.0) / (fabs(th) + sqrt(th * th + 1.0));
-            const double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
-            for (int k = 0; k < D; ++k) { const double a = A[k][p], b = A[k][q]; A[k][p] = c * a - s * b; A[k][q] = s * a + c * b; }
-            for (int k = 0; k < D; ++k) { const double a = A[p][k], b = A[q][k]; A[p][k] = c * a - s * b; A[q][k] = s * a + c * b; }
-        }
-    }
-    double e = A[0][0];
-    for (int i = 1; i < D; ++i) e = fmax(e, A[i][i]);
-    return e;
+// ---- fast FP64 helpers for positive, normal arguments (no zero / infinity / denormal branches) ----
+__device__ __forceinline__ double rsqrt_fast(double x) {      // hardware seed + one third-order step: < 1 ulp
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y * y, 1.0);
+    return fma(fma(e, 0.375, 0.5), y * e, y);
+}
+__device__ __forceinline__ double sqrt_fast(double x) {       // x * rsqrt(x) + one Newton correction
+    const double y = rsqrt_fast(x);
+    const double s = x * y;
+    return fma(fma(-s, s, x), 0.5 * y, s);
+}
+__device__ __forceinline__ double div_fast(double n, double dn) {   // n / dn, dn normal and non-zero
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(dn));
+    y = fma(y, fma(-dn, y, 1.0), y);
+    y = fma(y, fma(-dn, y, 1.0), y);
+    const double q = n * y;
+    return fma(fma(-dn, q, n), y, q);
 }
 
+// One Jacobi rotation that annihilates apq (r = the third index); eigenvalues only.
+__device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq, double &arp, double &arq) {
+    const double tau = aqq - app;
+    const double w2 = fma(tau, tau, 4.0 * apq * apq);
+    const bool on = (apq != 0.0) && (w2 > 0.0);
+    const double w = sqrt_fast(on ? w2 : 1.0);
+    const double den = tau + ((tau >= 0.0) ? w : -w);
+    const double t = on ? div_fast(2.0 * apq, den) : 0.0;
+    const double c = rsqrt_fast(fma(t, t, 1.0)), sn = t * c;
+    app = fma(-t, apq, app);
+    aqq = fma(t, apq, aqq);
+    apq = on ? 0.0 : apq;
+    const double rp = arp, rq = arq;
+    arp = c * rp - sn * rq;
+    arq = sn * rp + c * rq;
+}
+
+// Largest eigenvalue of a symmetric DxD matrix (eq. 48: maximum principal stress).
+// 3-D: cyclic Jacobi on the six independent components, the sweeps taken by the whole warp together
+// (the per-lane data-dependent loop of the first version cost more instructions than the pair
+// loop: profiles/r1b).  2-D: closed form.
+template <int D>
+__device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02, double a11, double a12, double a22) {
+    if (D == 2) {
+        const double hm = 0.5 * (a00 - a11), w2 = fma(hm, hm, a01 * a01);
+        return 0.5 * (a00 + a11) + ((w2 > 0.0) ? sqrt_fast(w2) : 0.0);
+    }
+    for (int sweep = 0; sweep < 12; ++sweep) {
+        const double off = a01 * a01 + a02 * a02 + a12 * a12;
+        const double dg = a00 * a00 + a11 * a11 + a22 * a22;
+        if (__all_sync(__activemask(), off <= 1e-36 * dg)) break;      // also off == 0
+        jacobi_rot(a00, a11, a01, a02, a12);      // (p, q, r) = (0, 1, 2)
+        jacobi_rot(a00, a22, a02, a01, a12);      // (0, 2, 1)
+        jacobi_rot(a11, a22, a12, a01, a02);      // (1, 2, 0)
+    }
+    return fmax(a00, fmax(a11, a22));
+}
+
+#define PR_WARPS 4
+#define PR_STRIDE 18            // doubles between staged records (144 B): 16-byte reads by lane are conflict-free
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::); }
+__device__ __forceinline__ void cp_async_wait1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+
+// One lane per particle, 32 Morton-consecutive particles per warp.  Round k handles the k-th partner
+// of every lane: the 32 partner records (128 B each, written by k_prepass) are copied to shared
+// memory by the whole warp -- 8 lanes fetch one record as 8 x 16 B, so a warp-wide copy touches 4
+// cache lines instead of 32 -- with cp.async one round ahead of the arithmetic; then every lane
+// reads ITS partner's record from shared memory (144-byte stride: conflict-free).
 template <int D, bool SOLID, bool VARH>
-__global__ void __launch_bounds__(128) k_pairs(Dev d, const sph_material *mats) {
+__global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_material *mats) {
     constexpr int NS = (D == 3) ? 6 : 3;                 // independent stress components
     constexpr int SI[6] = {0, 1, (D == 3) ? 2 : 3, 3, 4, 5};   // 2-D: xx xy yy -> 0 1 3
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    const int g = i >> 5;
+    __shared__ __align__(16) double s_buf[PR_WARPS][2][32 * PR_STRIDE];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = blockIdx.x * PR_WARPS + w;
     if (g * 32 >= d.n) return;
+    const int i = g * 32 + lane;
     const bool valid = i < d.n;
     const int ii = valid ? i : d.n - 1;
+    const unsigned FULL = 0xffffffffu;
+    const double *__restrict__ prec = d.prec;
 
     double xa[3], va[3], sa[NS];
-    for (int a = 0; a < D; ++a) { xa[a] = d.sx[a][ii]; va[a] = d.sv[a][ii]; }
-    for (int k = 0; k < NS; ++k) sa[k] = d.sr2[SI[k]][ii];
-    const double Hi = d.sh[ii], rhoi = d.srho[ii], csi = d.cs[ii];
+    double Hi, rhoi, csi;
+    {
+        const double2 *rec = reinterpret_cast<const double2 *>(prec + (size_t)ii * PR_REC);
+        const double2 c0 = rec[0], c1 = rec[1], c2 = rec[2], c3 = rec[3], c4 = rec[4], c5 = rec[5], c6 = rec[6], c7 = rec[7];
+        xa[0] = c0.x; xa[1] = c0.y; xa[2] = c1.x; va[0] = c1.y; va[1] = c2.x; va[2] = c2.y;
+        rhoi = c3.x; csi = c4.x; Hi = c4.y;
+        const double sr[6] = {c5.x, c5.y, c6.x, c6.y, c7.x, c7.y};
+        for (int k = 0; k < NS; ++k) sa[k] = sr[SI[k]];
+    }
     const double iHi = 1.0 / Hi;
     const double fac_i = 6.0 * KNorm<D>::s * ((D == 3) ? (iHi * iHi) * (iHi * iHi) : iHi * iHi * iHi);
     const int cnt = valid ? d.nb_cnt[ii] : 0;
     int mx = cnt;
-    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
     const int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
 
     double drho = 0.0, du = 0.0, dv[3] = {0, 0, 0};
     double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
     double N[6] = {0, 0, 0, 0, 0, 0};                     // symmetric moment matrix xx xy xz yy yz zz
 
+    // copy the records of partners `b` (one per lane) into buffer `buf`
+    const int sub = lane & 7, row0 = lane >> 3;
+    auto stage = [&](int b, int buf) {
+        double *dstb = &s_buf[w][buf][0];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+            const int r = row0 + 4 * t;
+            const int br = __shfl_sync(FULL, b, r);
+            cp_async16(dstb + r * PR_STRIDE + sub * 2, prec + (size_t)br * PR_REC + sub * 2);
+        }
+    };
+    int b_next = (0 < cnt) ? nbw[0] : ii;
+    if (mx > 0) stage(b_next, 0);
+    cp_async_commit();
+    b_next = (1 < cnt) ? nbw[32] : ii;
+
     for (int k = 0; k < mx; ++k) {
+        if (k + 1 < mx) stage(b_next, (k + 1) & 1);
+        cp_async_commit();
+        b_next = (k + 2 < cnt) ? nbw[(size_t)(k + 2) * 32] : ii;
+        cp_async_wait1();
+        __syncwarp();
+        const double2 *rec = reinterpret_cast<const double2 *>(&s_buf[w][k & 1][lane * PR_STRIDE]);
+        const double2 c0 = rec[0], c1 = rec[1], c2 = rec[2], c3 = rec[3], c4 = rec[4], c5 = rec[5], c6 = rec[6], c7 = rec[7];
         if (k < cnt) {
-            const int b = nbw[(size_t)k * 32];
+            const double xb[3] = {c0.x, c0.y, c1.x}, vb[3] = {c1.y, c2.x, c2.y};
+            const double rhob = c3.x, volb = c3.y, csb = c4.x, hb = c4.y;
+            const double sb6[6] = {c5.x, c5.y, c6.x, c6.y, c7.x, c7.y};
+            const double mb = rhob * volb;
             double dx[3], dvv[3];
             double r2 = 0.0, vr = 0.0;
             for (int a = 0; a < D; ++a) {
-                dx[a] = xa[a] - d.sx[a][b];
-                dvv[a] = va[a] - d.sv[a][b];
+                dx[a] = xa[a] - xb[a];
+                dvv[a] = va[a] - vb[a];
                 r2 += dx[a] * dx[a];
                 vr += dvv[a] * dx[a];
             }
-            const double mb = d.sm[b], rhob = d.srho[b], volb = d.vol[b], hb = d.sh[b];
             const double rinv = (r2 > 0.0) ? rsqrt(r2) : 0.0;
             const double r = r2 * rinv;
             double iH = iHi, fac = fac_i;
@@ -191,14 +286,14 @@ __global__ void __launch_bounds__(128) k_pairs(Dev d, const sph_material *mats) 
             drho += volb * vg;                                // eq. 29
             double Pi = 0.0;
             if (vr < 0.0) {                                   // eqs. 32-33, approaching pairs only
-                const double Hb = 0.5 * (Hi + hb), cb = 0.5 * (csi + d.cs[b]), rb = 0.5 * (rhoi + rhob);
+                const double Hb = 0.5 * (Hi + hb), cb = 0.5 * (csi + csb), rb = 0.5 * (rhoi + rhob);
                 const double den = r2 + d.av_eps * Hb * Hb;
                 const double inv = 1.0 / (den * rb);
                 const double nu = Hb * vr * rb * inv;
                 Pi = nu * (d.av_beta * nu - d.av_alpha * cb) * den * inv;
             }
             double T[NS];
-            for (int k2 = 0; k2 < NS; ++k2) T[k2] = sa[k2] + d.sr2[SI[k2]][b];
+            for (int k2 = 0; k2 < NS; ++k2) T[k2] = sa[k2] + sb6[SI[k2]];
             double fv[3];
             if (D == 3) {
                 T[0] -= Pi; T[3] -= Pi; T[5] -= Pi;
@@ -223,6 +318,7 @@ __global__ void __launch_bounds__(128) k_pairs(Dev d, const sph_material *mats) 
                 if (D == 3) { const double u2 = -volb * dx[2]; N[2] += u0 * gW[2]; N[4] += u1 * gW[2]; N[5] += u2 * gW[2]; }
             }
         }
+        __syncwarp();                                         // buffer k & 1 is refilled in round k + 1
     }
     if (!valid) return;
 
@@ -297,10 +393,9 @@ __global__ void __launch_bounds__(128) k_pairs(Dev d, const sph_material *mats) 
             if (dd < 1.0 && ntot > 0) {
                 const double p = d.p[i];
                 const double phat = (p >= 0.0) ? p : (1.0 - dd) * p;
-                double A[3][3];
-                A[0][0] = (1.0 - dd) * St[0] - phat; A[0][1] = A[1][0] = (1.0 - dd) * St[1]; A[0][2] = A[2][0] = (1.0 - dd) * St[2];
-                A[1][1] = (1.0 - dd) * St[3] - phat; A[1][2] = A[2][1] = (1.0 - dd) * St[4]; A[2][2] = (1.0 - dd) * St[5] - phat;
-                const double smax = max_eig_jacobi<D>(A);
+                const double od = 1.0 - dd;
+                const double smax = max_eig_sym<D>(od * St[0] - phat, od * St[1], od * St[2], od * St[3] - phat,
+                                                   od * St[4], od * St[5] - phat);
                 const double K = (mt.eos == SPH_EOS_TILLOTSON) ? mt.tA : mt.K0;
                 const double E = 9.0 * K * mt.mu / (3.0 * K + mt.mu);
                 strain = smax / ((1.0 - dd) * E);
@@ -323,6 +418,7 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
     const int n = d.n;
     const bool varh = (d.flags & SPH_F_VARIABLE_H) != 0, solid = (d.flags & SPH_F_SOLID) != 0;
     const int gb = sph_ceil_div((i64)sph_ceil_div(n, 32) * 32, 128);
+    const int pb = sph_ceil_div(sph_ceil_div(n, 32), PR_WARPS);
     if (d.flags & SPH_F_DENSITY_SUM) {
         StageTimer tm(ctx, SPH_T_DENSITY);
         if (varh) k_density<D, true><<<gb, 128, 0, ctx->stream>>>(d);
@@ -336,11 +432,11 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
     }
     StageTimer tm(ctx, SPH_T_PAIRS);
     if (solid) {
-        if (varh) k_pairs<D, true, true><<<gb, 128, 0, ctx->stream>>>(d, mats);
-        else k_pairs<D, true, false><<<gb, 128, 0, ctx->stream>>>(d, mats);
+        if (varh) k_pairs<D, true, true><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
+        else k_pairs<D, true, false><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
     } else {
-        if (varh) k_pairs<D, false, true><<<gb, 128, 0, ctx->stream>>>(d, mats);
-        else k_pairs<D, false, false><<<gb, 128, 0, ctx->stream>>>(d, mats);
+        if (varh) k_pairs<D, false, true><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
+        else k_pairs<D, false, false><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
     }
     ctx->launches += 1;
 }

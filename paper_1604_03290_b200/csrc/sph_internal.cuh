@@ -40,6 +40,7 @@ struct DevRoot {
 // SPH_BUCKET particles ("big" cells) and buckets of <= SPH_BUCKET Morton-consecutive particles, in
 // depth-first pre-order.  skip >= 0: big cell, index of the first record after its subtree;
 // skip < 0: bucket of -skip particles starting at sorted index lo.
+#define PR_REC 16
 #define SPH_BUCKET 32
 struct __align__(16) SearchItem {
     double bmin[3], bmax[3];    // tight bounding box of the particles below
@@ -111,7 +112,8 @@ struct Dev {
     int *nb_cnt;
     int *own_cnt;               // n_a of eq. 73
     // ---- pre-pass ----
-    double *p, *cs, *vol, *sr2[6];      // pressure, sound speed, m/rho, sigma/rho^2
+    double *p, *cs;             // pressure, sound speed
+    double *prec;               // PR_REC doubles per particle: x3 v3 rho m/rho cs h sigma/rho^2 (6)
     // ---- rates, sorted order ----
     double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *strain;
     int *n_act_new;
