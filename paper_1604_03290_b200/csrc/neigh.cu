@@ -224,23 +224,6 @@ __global__ void k_writeback_h(Dev d) {
     d.h[d.perm[i]] = d.sh[i];
 }
 
-// hmax of every cell must follow the new h (hmax only; the boxes are unchanged)
-__global__ void k_hmax(Dev d, int level) {
-    const int nd = blockIdx.x * blockDim.x + threadIdx.x;
-    if (nd >= d.status->n_nodes) return;
-    if (d.nlevel[nd] != level) return;
-    const int NC = 1 << d.D;
-    const int *cl = d.child_lo + (size_t)nd * (NC + 1);
-    const int *ch = d.child + (size_t)nd * NC;
-    double hmax = 0.0;
-    for (int c = 0; c < NC; ++c) {
-        const int code = ch[c];
-        if (code >= 0) hmax = fmax(hmax, d.nhmax[code]);
-        else if (code == -2) for (int p = cl[c]; p < cl[c + 1]; ++p) hmax = fmax(hmax, d.sh[p]);
-    }
-    d.nhmax[nd] = hmax;
-}
-
 template <int D>
 static void launch_neigh(sph_ctx *ctx, bool varh, bool count_only) {
     Dev &d = ctx->d;
@@ -267,10 +250,7 @@ void sph_stage_neigh(sph_ctx *ctx) {
             if (d.D == 3) launch_neigh<3>(ctx, varh, true); else launch_neigh<2>(ctx, varh, true);
             k_h_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
             ctx->launches += 1;
-            for (int lvl = d.L - 1; lvl >= 0; --lvl) {
-                k_hmax<<<sph_ceil_div(d.n, 128), 128, 0, ctx->stream>>>(d, lvl);
-                ctx->launches += 1;
-            }
+            sph_launch_moments(ctx, 1);      // hmax of every cell follows the new h (the boxes are unchanged)
             emit_items(ctx);                 // refresh hmax of the records
         }
         sph_stage_writeback_h(ctx);

@@ -168,10 +168,10 @@ __device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq
 // loop: profiles/r1b).  2-D: closed form.
 template <int D>
 __device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02, double a11, double a12, double a22) {
-    if (D == 2) {
+    if constexpr (D == 2) {
         const double hm = 0.5 * (a00 - a11), w2 = fma(hm, hm, a01 * a01);
         return 0.5 * (a00 + a11) + ((w2 > 0.0) ? sqrt_fast(w2) : 0.0);
-    }
+    } else {
     for (int sweep = 0; sweep < 12; ++sweep) {
         const double off = a01 * a01 + a02 * a02 + a12 * a12;
         const double dg = a00 * a00 + a11 * a11 + a22 * a22;
@@ -181,6 +181,7 @@ __device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02
         jacobi_rot(a11, a22, a12, a01, a02);      // (1, 2, 0)
     }
     return fmax(a00, fmax(a11, a22));
+    }
 }
 
 #define PR_WARPS 4

@@ -96,6 +96,7 @@ struct Dev {
     int *nhi[2];
     int *nlevel, *nlo, *nhi_s;  // per node
     int *nskip;                 // first node after the subtree (pre-order)
+    int *nparent, *ncc, *nready; // parent cell (-1 root), number of child CELLS, children finished (k_moments)
     int *child;                 // NC per node: >=0 node, -1 empty, -2 leaf
     int *child_lo;              // NC+1 per node
     double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
@@ -170,6 +171,7 @@ void sph_stage_rhs(sph_ctx *ctx);       // A6-A10
 void sph_stage_gravity(sph_ctx *ctx);   // A11
 void sph_stage_update(sph_ctx *ctx, double c, int commit);   // A12 (one of the two updates)
 void sph_stage_writeback_h(sph_ctx *ctx);
+void sph_launch_moments(sph_ctx *ctx, int hmax_only);   // tree.cu: pseudo-particles bottom-up, one launch
 
 // ---- exact-order arithmetic for the floating-point decisions (never contracted to FMA) ----
 __device__ __forceinline__ double sph_r2_exact(double dx, double dy, double dz, int D) {

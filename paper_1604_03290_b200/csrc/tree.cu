@@ -10,8 +10,8 @@
 //   radix sort   : nodes sorted by (lo, level)  == depth-first (pre-order) numbering
 //   k_fill_nodes : child boundaries by binary search in the node's key range; child node ids by
 //                  binary search in the sorted node keys
-//   k_moments    : one launch per level, deepest first: mass, centre of mass (monopole only,
-//                  PAPER.md:370, :380, :473-475), tight bounding box and hmax.  Children are
+//   k_moments    : ONE launch, threads climb from the deepest cells: mass, centre of mass (monopole
+//                  only), tight bounding box and hmax.  Children are
 //                  summed in octant order, every operation rounded separately (reading U15), so
 //                  that the opening decisions of the gravity walk are reproducible bit for bit.
 #include "sph_internal.cuh"
@@ -87,6 +87,9 @@ __global__ void k_fill_nodes(Dev d, const u64 *__restrict__ nkey, const int *__r
     int *cl = d.child_lo + (size_t)nd * (NC + 1);
     int *ch = d.child + (size_t)nd * NC;
     cl[0] = lo;
+    int ncc = 0;
+    if (nd == 0) d.nparent[0] = -1;
+    d.nready[nd] = 0;
     for (int c = 0; c < NC; ++c) {
         int e = (c == NC - 1) ? hi : lower_bound_key(d.keys, b, hi, ((prefix << D) | (u64)(c + 1)) << (shift - D));
         cl[c + 1] = e;
@@ -101,16 +104,19 @@ __global__ void k_fill_nodes(Dev d, const u64 *__restrict__ nkey, const int *__r
             int l2 = nd + 1, h2 = nn;                       // children follow their parent in pre-order
             while (l2 < h2) { int mid = (l2 + h2) >> 1; if (nkey[mid] < want) l2 = mid + 1; else h2 = mid; }
             code = l2;
+            d.nparent[l2] = nd;
+            ++ncc;
         }
         ch[c] = code;
         b = e;
     }
+    d.ncc[nd] = ncc;
 }
 
-__global__ void k_moments(Dev d, int level) {
-    const int nd = blockIdx.x * blockDim.x + threadIdx.x;
-    if (nd >= d.status->n_nodes) return;
-    if (d.nlevel[nd] != level) return;
+// Pseudo-particle of one cell from its children, children in octant order, every
+// operation rounded separately (reading U15).  Child cells are read with ld.global.cg: they were
+// written by other threads of the same launch.
+__device__ __forceinline__ void cell_moments(const Dev &d, int nd, bool hmax_only) {
     const int D = d.D, NC = 1 << D;
     const int *cl = d.child_lo + (size_t)nd * (NC + 1);
     const int *ch = d.child + (size_t)nd * NC;
@@ -120,16 +126,19 @@ __global__ void k_moments(Dev d, int level) {
         const int code = ch[c];
         if (code == -1) continue;
         if (code >= 0) {
-            const double mc = d.nmass[code];
+            hmax = fmax(hmax, __ldcg(&d.nhmax[code]));
+            if (hmax_only) continue;
+            const double mc = __ldcg(&d.nmass[code]);
             M = __dadd_rn(M, mc);
             for (int a = 0; a < D; ++a) {
-                S[a] = __dadd_rn(S[a], __dmul_rn(mc, d.ncom[a][code]));
-                bmin[a] = fmin(bmin[a], d.nbmin[a][code]);
-                bmax[a] = fmax(bmax[a], d.nbmax[a][code]);
+                S[a] = __dadd_rn(S[a], __dmul_rn(mc, __ldcg(&d.ncom[a][code])));
+                bmin[a] = fmin(bmin[a], __ldcg(&d.nbmin[a][code]));
+                bmax[a] = fmax(bmax[a], __ldcg(&d.nbmax[a][code]));
             }
-            hmax = fmax(hmax, d.nhmax[code]);
         } else {
             for (int p = cl[c]; p < cl[c + 1]; ++p) {
+                hmax = fmax(hmax, d.sh[p]);
+                if (hmax_only) continue;
                 const double mp = d.sm[p];
                 M = __dadd_rn(M, mp);
                 for (int a = 0; a < D; ++a) {
@@ -138,17 +147,53 @@ __global__ void k_moments(Dev d, int level) {
                     bmin[a] = fmin(bmin[a], xp);
                     bmax[a] = fmax(bmax[a], xp);
                 }
-                hmax = fmax(hmax, d.sh[p]);
             }
         }
     }
+    d.nhmax[nd] = hmax;
+    if (hmax_only) return;
     d.nmass[nd] = M;
     for (int a = 0; a < 3; ++a) {
         d.ncom[a][nd] = (a < D) ? __ddiv_rn(S[a], M) : 0.0;
         d.nbmin[a][nd] = (a < D) ? bmin[a] : 0.0;
         d.nbmax[a][nd] = (a < D) ? bmax[a] : 0.0;
     }
-    d.nhmax[nd] = hmax;
+}
+
+// Bottom-up in ONE launch (the first version launched once per level: 21 launches, 0.75 ms on C5).
+// A thread starts at a cell without child cells and climbs: after finishing a cell it increments
+// the parent's counter; the thread that brings the counter to the parent's number of child cells
+// computes the parent (all its children are complete and visible: fence before the increment),
+// the others retire.  The arithmetic of a cell does not depend on which thread performs it.
+__global__ void k_moments(Dev d, int hmax_only) {
+    int nd = blockIdx.x * blockDim.x + threadIdx.x;
+    if (nd >= d.status->n_nodes) return;
+    if (d.ncc[nd] != 0) return;
+    while (true) {
+        cell_moments(d, nd, hmax_only != 0);
+        const int parent = d.nparent[nd];
+        if (parent < 0) return;
+        __threadfence();
+        const int done = atomicAdd(&d.nready[parent], 1) + 1;
+        if (done != d.ncc[parent]) return;
+        __threadfence();
+        nd = parent;
+    }
+}
+
+__global__ void k_reset_ready(Dev d) {
+    const int nd = blockIdx.x * blockDim.x + threadIdx.x;
+    if (nd < d.status->n_nodes) d.nready[nd] = 0;
+}
+
+void sph_launch_moments(sph_ctx *ctx, int hmax_only) {
+    Dev &d = ctx->d;
+    if (hmax_only) {            // a second climb over the same tree: the counters start from zero again
+        k_reset_ready<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
+        ctx->launches += 1;
+    }
+    k_moments<<<sph_ceil_div(d.n, 128), 128, 0, ctx->stream>>>(d, hmax_only);
+    ctx->launches += 1;
 }
 
 __global__ void k_zero_status(Dev d) {
@@ -171,8 +216,5 @@ void sph_stage_tree(sph_ctx *ctx) {
     ctx->launches += 1;
     delete tt;
     StageTimer tm(ctx, SPH_T_MOMENTS);
-    for (int lvl = d.L - 1; lvl >= 0; --lvl) {
-        k_moments<<<sph_ceil_div(n, 128), 128, 0, ctx->stream>>>(d, lvl);
-        ctx->launches += 1;
-    }
+    sph_launch_moments(ctx, 0);
 }

@@ -1,0 +1,114 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same config_of,
+same sph_evaluate): the oracle cannot evaluate millions of particles by brute force, so
+  * Morton keys and permutation are compared for ALL particles (bit-exact), the octree node list
+    (level, prefix, range) and the pseudo-particle moments for ALL nodes (bit-exact);
+  * partner lists and every FP64 rate are compared on a seeded SAMPLE of target particles that the
+    oracle evaluates one by one in its tree mode (its own reference tree; pinned against brute force
+    in tests/test_oracle_pins.py), sets bit-exact, rates within T1;
+  * properties that hold at any size: partner counts of the lattice interior, total momentum of the
+    SPH forces, finite outputs.
+Twins are used (every branch of the rate equations active on every particle); the nominal inputs
+have exactly zero SPH rates almost everywhere at t = 0.
+"""
+import numpy as np
+import pytest
+
+import sph_inputs
+from oracle import oracle as orc
+from test_gpu_parity import P, assert_close, canonical, check_rates, make_ctx  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+N_SAMPLE = 1500
+
+
+def _sample(w, seed):
+    rng = np.random.default_rng(seed)
+    t = rng.choice(w.n, min(N_SAMPLE, w.n), replace=False)
+    # always include the first/last particles in Morton order's ragged tail and the extremes of x
+    extra = np.array([0, w.n - 1, int(np.argmin(w.x[0])), int(np.argmax(w.x[0]))])
+    return np.unique(np.concatenate([t, extra])).astype(np.int64)
+
+
+def _full_case(P, w, seed):
+    ctx = make_ctx(P, w, h_iters=0)
+    ctx.evaluate()
+    ctx.sync()
+    # ---- order and tree: all particles, all nodes ----
+    tree = orc.Tree(w)
+    okey, operm = tree.order()
+    keys, perm, root = ctx.get_order()
+    assert np.array_equal(keys, okey), "Morton keys differ"
+    assert np.array_equal(perm, operm), "permutation differs"
+    assert root[3] == tree.s0
+    on = tree.nodes()
+    gn = canonical(ctx.get_tree())
+    assert gn["level"].size == on["level"].size, "node count differs"
+    for k in ("level", "prefix", "lo", "hi"):
+        assert np.array_equal(gn[k], on[k]), f"tree {k} differs"
+    for k in ("mass", "hmax"):
+        assert np.array_equal(gn[k], on[k]), f"node {k} differs"
+    for k in ("com", "bmin", "bmax"):
+        assert np.array_equal(gn[k][:, :w.dim], on[k][:, :w.dim]), f"node {k} differs"
+    # ---- sampled targets: partner sets and rates ----
+    t = _sample(w, seed)
+    o = orc.evaluate(w, mode="tree", targets=t, h_iters=0)
+    off, idx = ctx.get_neighbours()
+    for k, a in enumerate(t):
+        assert np.array_equal(idx[off[a]:off[a + 1]], o["nb_idx"][o["nb_off"][k]:o["nb_off"][k + 1]]), \
+            f"partner set of particle {a} differs"
+    g = ctx.download()
+    assert np.array_equal(g["nb_count"], np.diff(off))
+    check_rates(w, g, o, targets=t)
+    # ---- properties at any size ----
+    for k in ("drho", "du", "dv", "dS", "ag", "ddmg"):
+        assert np.all(np.isfinite(g[k])), k
+    mom = (w.m[None, :] * g["dv"]).sum(axis=1)
+    scale = (w.m[None, :] * np.abs(g["dv"])).sum(axis=1).max()
+    assert np.all(np.abs(mom) <= 1e-11 * scale), "pairwise SPH forces do not cancel"
+    c = ctx.get_counters()
+    assert c["n_pairs"] == int(off[-1])
+    if w.flags & orc.F_GRAVITY:
+        assert c["n_inter"] > 0
+        # sampled interaction counts: the accepted set of every sampled particle has the oracle's size
+        assert o["n_inter"].min() > 0
+    ctx.close()
+    return g, off
+
+
+def test_c2_full_size(P):
+    w = sph_inputs.make("C2", twin=True)                     # 65 536 particles, variable h, gravity
+    _full_case(P, w, 21)
+
+
+def test_c3_full_size(P):
+    w = sph_inputs.make("C3", twin=True)                     # 493 290 particles
+    g, off = _full_case(P, w, 22)
+    # lattice interior: exactly 80 partners (tests/golden/lattice_sums.txt)
+    assert np.bincount(np.diff(off)).argmax() == 80
+
+
+def test_c4_full_size(P):
+    w = sph_inputs.make("C4", twin=True)                     # 2.0 M particles, 33 M flaws
+    g, off = _full_case(P, w, 23)
+    assert np.bincount(np.diff(off)).argmax() == 80
+
+
+def test_c5_full_size(P):
+    w = sph_inputs.make("C5", twin=True)                     # 4.0 M particles, gravity, damage
+    g, off = _full_case(P, w, 24)
+    assert np.bincount(np.diff(off)).argmax() == 80
+    # every particle of a body is pulled towards the pair's common centre of mass region: no zero rows
+    assert np.all(np.abs(g["ag"]).sum(axis=0) > 0.0)
+
+
+def test_c1_full_size(P):
+    w = sph_inputs.make("C1", twin=True)                     # 4 398 particles: brute force is affordable
+    ctx = make_ctx(P, w, h_iters=0)
+    ctx.evaluate()
+    o = orc.evaluate(w, mode="brute", h_iters=0)
+    off, idx = ctx.get_neighbours()
+    assert np.array_equal(off, o["nb_off"]) and np.array_equal(idx, o["nb_idx"])
+    check_rates(w, ctx.download(), o)
+    assert np.bincount(np.diff(off)).argmax() == 20
+    ctx.close()
