@@ -117,18 +117,30 @@ __global__ void k_sort_hist(const u64 *__restrict__ kin, int n_host, const int *
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
+// Stable scatter of one 8-bit digit.  Ranks inside a warp come from match_any; the tile is first
+// put into digit order in shared memory, so that consecutive threads write consecutive addresses
+// of the output (runs of one digit) instead of 256 scattered streams.
+struct SortSmem {
+    u64 key[SORT_TILE];
+    int val[SORT_TILE];
+    unsigned wc[SORT_WARPS][256];
+    unsigned gbase[256];        // global start of the tile's run of every digit
+    unsigned lstart[256];       // start of the digit inside the tile
+};
+
 __global__ void __launch_bounds__(SORT_THREADS)
 k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__restrict__ kout,
                int *__restrict__ vout, int n_host, const int *n_dev, int shift,
                const unsigned *__restrict__ offs, int nblocks) {
-    __shared__ unsigned wc[SORT_WARPS][256];
-    __shared__ unsigned gbase[256];
+    extern __shared__ __align__(16) unsigned char sort_raw[];
+    SortSmem &sm = *reinterpret_cast<SortSmem *>(sort_raw);
     const int n = n_dev ? *n_dev : n_host;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int k = threadIdx.x; k < SORT_WARPS * 256; k += SORT_THREADS) (&wc[0][0])[k] = 0;
-    gbase[threadIdx.x] = offs[threadIdx.x * nblocks + blockIdx.x];
+    for (int k = threadIdx.x; k < SORT_WARPS * 256; k += SORT_THREADS) (&sm.wc[0][0])[k] = 0;
+    sm.gbase[threadIdx.x] = offs[threadIdx.x * nblocks + blockIdx.x];
     __syncthreads();
-    const i64 base = (i64)blockIdx.x * SORT_TILE + (i64)w * (32 * SORT_ITEMS);
+    const i64 tile0 = (i64)blockIdx.x * SORT_TILE;
+    const i64 base = tile0 + (i64)w * (32 * SORT_ITEMS);
     u64 key[SORT_ITEMS];
     int val[SORT_ITEMS];
     unsigned rank[SORT_ITEMS];
@@ -141,16 +153,29 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
         val[j] = valid ? vin[i] : 0;
         unsigned dg = (unsigned)(key[j] >> shift) & 255u;
         unsigned m = __match_any_sync(0xffffffffu, valid ? dg : 256u);
-        unsigned prev = valid ? wc[w][dg] : 0u;
+        unsigned prev = valid ? sm.wc[w][dg] : 0u;
         __syncwarp();
-        if (valid && (m & lt) == 0) wc[w][dg] = prev + __popc(m);
+        if (valid && (m & lt) == 0) sm.wc[w][dg] = prev + __popc(m);
         __syncwarp();
         rank[j] = prev + __popc(m & lt);
     }
     __syncthreads();
-    {   // exclusive scan over warps, one digit per thread
+    unsigned tot;
+    {   // exclusive scan over warps, one digit per thread; then over the digits of the tile
         unsigned run = 0;
-        for (int k = 0; k < SORT_WARPS; ++k) { unsigned t = wc[k][threadIdx.x]; wc[k][threadIdx.x] = run; run += t; }
+        for (int k = 0; k < SORT_WARPS; ++k) { unsigned t = sm.wc[k][threadIdx.x]; sm.wc[k][threadIdx.x] = run; run += t; }
+        tot = run;
+    }
+    {
+        unsigned inc = tot;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+        __shared__ unsigned wsum[SORT_WARPS];
+        if (lane == 31) wsum[w] = inc;
+        __syncthreads();
+        unsigned off = 0;
+        for (int k = 0; k < w; ++k) off += wsum[k];
+        sm.lstart[threadIdx.x] = off + inc - tot;
     }
     __syncthreads();
 #pragma unroll
@@ -158,20 +183,34 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
         i64 i = base + j * 32 + lane;
         if (i < n) {
             unsigned dg = (unsigned)(key[j] >> shift) & 255u;
-            unsigned pos = gbase[dg] + wc[w][dg] + rank[j];
-            kout[pos] = key[j];
-            vout[pos] = val[j];
+            unsigned lp = sm.lstart[dg] + sm.wc[w][dg] + rank[j];
+            sm.key[lp] = key[j];
+            sm.val[lp] = val[j];
         }
+    }
+    __syncthreads();
+    const int cnt = (int)min((i64)SORT_TILE, (i64)n - tile0);
+    for (int k = threadIdx.x; k < cnt; k += SORT_THREADS) {
+        const u64 kk = sm.key[k];
+        const unsigned dg = (unsigned)(kk >> shift) & 255u;
+        const unsigned pos = sm.gbase[dg] + ((unsigned)k - sm.lstart[dg]);
+        kout[pos] = kk;
+        vout[pos] = sm.val[k];
     }
 }
 
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur) {
     const int nblocks = sph_ceil_div(n_host, SORT_TILE);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        attr_set = true;
+    }
     int c = *cur;
     for (int shift = 0; shift < bits; shift += 8) {
         k_sort_hist<<<nblocks, 256, 0, ctx->stream>>>(key[c], n_host, n_dev, shift, ctx->d.hist, nblocks);
         sph_scan_u32(ctx, ctx->d.hist, ctx->d.hist, (i64)256 * nblocks, (unsigned *)ctx->d.scan_tmp);
-        k_sort_scatter<<<nblocks, SORT_THREADS, 0, ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host,
+        k_sort_scatter<<<nblocks, SORT_THREADS, sizeof(SortSmem), ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host,
                                                                   n_dev, shift, ctx->d.hist, nblocks);
         ctx->launches += 2;
         c ^= 1;
