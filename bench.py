@@ -223,7 +223,7 @@ def run_ours(args, rank, world):
 
 
 def sph_inputs_seed(name):
-    return {"C1": 1604, "C2": 1605, "C3": 1606, "C4": 1607, "C5": 1608}[name]
+    return {"C1": 1604, "C1x": 1604, "C2": 1605, "C3": 1606, "C4": 1607, "C5": 1608}[name]
 
 
 # ---------------------------------------------------------------------------------------------

@@ -52,7 +52,9 @@ enum {
     SPH_F_DAMAGE = 4,        /* Grady-Kipp damage */
     SPH_F_GRAVITY = 8,       /* Barnes-Hut self-gravity */
     SPH_F_VARIABLE_H = 16,   /* mean smoothing length per pair + eq. 73 update */
-    SPH_F_DENSITY_SUM = 32   /* rho by kernel sum, eq. 28, instead of continuity */
+    SPH_F_DENSITY_SUM = 32,  /* rho by kernel sum, eq. 28, instead of continuity */
+    SPH_F_ART_STRESS = 64,   /* artificial stress against the tensile instability (eqs. 35-38) */
+    SPH_F_XSPH = 128         /* particles move with the XSPH-smoothed velocity (eq. 40) */
 };
 
 enum { SPH_EOS_IDEAL_GAS = 0, SPH_EOS_MURNAGHAN = 1, SPH_EOS_TILLOTSON = 2 };
@@ -83,6 +85,9 @@ typedef struct {
     double G;               /* gravitational constant */
     double eps_soft;        /* Plummer softening length added in eq. 51 */
     double av_alpha, av_beta, av_eps; /* artificial viscosity, eqs. 32-33 */
+    double as_eps, as_n, as_mpd;      /* artificial stress: factor eps_s (eq. 37), exponent n and mean particle
+                                         distance dmpd of f = W(r)/W(dmpd) (eq. 38); used with SPH_F_ART_STRESS */
+    double xsph;                      /* XSPH factor x_sph of eq. 40; used with SPH_F_XSPH */
 } sph_config;
 
 /* Input state, original order.  NULL members are left unchanged (or zero on first upload).
@@ -99,11 +104,14 @@ typedef struct {
  * State: x, v, rho, u, S, dmg, h, n_act.  Rates of the LAST evaluation: drho (eq. 29), dv (eqs. 30/34,
  * SPH part only), du (eq. 31), dS (eqs. 7-10), ddmg (eq. 46, rate of dmg = d^(1/3)), ag (eq. 51,
  * gravitational acceleration), p and cs (equation of state), strain (eq. 48), n_act_new (activated
- * flaws found by the last evaluation, latched with the committed count), nb_count (partners). */
+ * flaws found by the last evaluation, latched with the committed count), nb_count (partners),
+ * dxs (eq. 40: the XSPH term x_sph sum_b 2 m_b/(rho_a+rho_b) (v_b - v_a) W_ab, so that dx/dt = v + dxs;
+ * zero without SPH_F_XSPH). */
 typedef struct {
     double *x[3], *v[3], *rho, *u, *S[6], *dmg, *h;
     double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *p, *cs, *strain;
     int32_t *n_act, *n_act_new, *nb_count;
+    double *dxs[3];
 } sph_state_out;
 
 /* Bytes of device workspace sph_create needs for this configuration (0 on invalid config). */

@@ -17,6 +17,7 @@ import numpy as np
 from . import build as _build
 
 F_SOLID, F_PLASTIC, F_DAMAGE, F_GRAVITY, F_VARIABLE_H, F_DENSITY_SUM = 1, 2, 4, 8, 16, 32
+F_ART_STRESS, F_XSPH = 64, 128
 
 _P = C.POINTER
 _dp = _P(C.c_double)
@@ -34,7 +35,8 @@ class Cfg(C.Structure):
     _fields_ = [("dim", C.c_int), ("flags", C.c_int), ("L", C.c_int), ("n_materials", C.c_int),
                 ("n", C.c_longlong), ("theta", C.c_double), ("G", C.c_double),
                 ("eps_soft", C.c_double), ("av_alpha", C.c_double), ("av_beta", C.c_double),
-                ("av_eps", C.c_double)]
+                ("av_eps", C.c_double), ("as_eps", C.c_double), ("as_n", C.c_double),
+                ("as_mpd", C.c_double), ("xsph", C.c_double)]
 
 
 class State(C.Structure):
@@ -47,7 +49,7 @@ class Rates(C.Structure):
     _fields_ = [("drho", _dp), ("dv", _dp * 3), ("du", _dp), ("gradv", _dp * 9), ("dS", _dp * 6),
                 ("ddmg", _dp), ("strain", _dp), ("C", _dp * 9), ("n_act", _ip),
                 ("A_drho", _dp), ("A_dv", _dp * 3), ("A_du", _dp), ("A_gradv", _dp * 9),
-                ("A_dS", _dp * 6)]
+                ("A_dS", _dp * 6), ("dxs", _dp * 3), ("A_dxs", _dp * 3)]
 
 
 _lib = None
@@ -141,7 +143,8 @@ class _Bound:
         self.n = w.n
         self.cfg = Cfg(dim=w.dim, flags=w.flags, L=L, n_materials=len(w.materials), n=w.n,
                        theta=w.theta, G=w.G, eps_soft=w.eps_soft, av_alpha=w.av_alpha,
-                       av_beta=w.av_beta, av_eps=w.av_eps)
+                       av_beta=w.av_beta, av_eps=w.av_eps, as_eps=w.as_eps, as_n=w.as_n,
+                       as_mpd=w.as_mpd, xsph=w.xsph)
         self.mats = make_mats(w.materials)
         st = State()
         x, v, S = _f64(w.x), _f64(w.v), _f64(w.S)
@@ -273,7 +276,8 @@ def rhs(w, off, idx, targets=None, rho=None, h=None, n_act=None):
     out = dict(drho=np.zeros(nt), dv=np.zeros((3, nt)), du=np.zeros(nt), gradv=np.zeros((9, nt)),
                dS=np.zeros((6, nt)), ddmg=np.zeros(nt), strain=np.zeros(nt), C=np.zeros((9, nt)),
                n_act=np.zeros(nt, np.int32), A_drho=np.zeros(nt), A_dv=np.zeros((3, nt)),
-               A_du=np.zeros(nt), A_gradv=np.zeros((9, nt)), A_dS=np.zeros((6, nt)))
+               A_du=np.zeros(nt), A_gradv=np.zeros((9, nt)), A_dS=np.zeros((6, nt)),
+               dxs=np.zeros((3, nt)), A_dxs=np.zeros((3, nt)))
     r = Rates()
     for k, _ in Rates._fields_:
         arr = out[k]
@@ -377,7 +381,10 @@ def step(w, dt, mode="brute"):
 
     def advance(base, vel, f, c, n_act_eval):
         q = base.copy()
-        q.x = base.x + c * vel                          # dx/dt = v (eq. 39)
+        if w.flags & F_XSPH:
+            q.x = base.x + c * (vel + f["dxs"])         # eq. 40
+        else:
+            q.x = base.x + c * vel                      # dx/dt = v (eq. 39)
         q.v = base.v + c * (f["dv"] + f["ag"])
         if w.flags & F_DENSITY_SUM:
             q.rho = f["rho"].copy()                     # not integrated: eq. 28 each evaluation

@@ -44,6 +44,7 @@ struct orc_cfg {
     int dim, flags, L, n_materials;
     i64 n;
     double theta, G, eps_soft, av_alpha, av_beta, av_eps;
+    double as_eps, as_n, as_mpd, xsph;   // artificial stress (eqs. 35-38) and XSPH factor (eq. 40)
 };
 
 struct orc_state {
@@ -57,9 +58,11 @@ struct orc_rates {                  // all arrays have one entry per TARGET
     double *drho, *dv[3], *du, *gradv[9], *dS[6], *ddmg, *strain, *C[9];
     int *n_act;
     double *A_drho, *A_dv[3], *A_du, *A_gradv[9], *A_dS[6];   // sums of |pair terms| (T1)
+    double *dxs[3], *A_dxs[3];      // XSPH velocity correction (eq. 40) and its sum of |terms|
 };
 
-enum { F_SOLID = 1, F_PLASTIC = 2, F_DAMAGE = 4, F_GRAVITY = 8, F_VARIABLE_H = 16, F_DENSITY_SUM = 32 };
+enum { F_SOLID = 1, F_PLASTIC = 2, F_DAMAGE = 4, F_GRAVITY = 8, F_VARIABLE_H = 16, F_DENSITY_SUM = 32,
+       F_ART_STRESS = 64, F_XSPH = 128 };
 
 // -------------------------------------------------------------------------------------
 // P1. Cubic B-spline kernel, PAPER.md:217 (eq. 25), :221 (eq. 26), :226 (eq. 27).
@@ -552,12 +555,16 @@ static bool invert(int D, const double N[3][3], double C[3][3], double *det_out)
 //   grad v       PAPER.md:317-330 (eqs. 41-44)    C = inverse of the (x_b - x_a) matrix (U6, U17)
 //   dS/dt        PAPER.md:83-96 (eqs. 7-10)       1/D in the trace term (U8)
 //   damage       PAPER.md:344-360 (eqs. 46-49), :189 (eq. 24 repaired, U16), U18-U20
+//   art. stress  PAPER.md:284-302 (eqs. 35-38)    zeta = -eps_s sigma/rho^2 per component in tension (U25),
+//                                                 f = W_ab / W(dmpd), same term in the energy sum (U3)
+//   XSPH         PAPER.md:311 (eq. 40)            2 m_b / (rho_a + rho_b) (U26)
 // -------------------------------------------------------------------------------------
 void orc_rhs(const orc_cfg *c, const orc_mat *mats, const orc_state *s, const double *p,
              const double *cs, const double *sigma, const double *St, i64 nt, const i64 *targets,
              const i64 *off, const int *idx, orc_rates *o) {
     const int D = c->dim;
     const bool solid = (c->flags & F_SOLID) != 0, varh = (c->flags & F_VARIABLE_H) != 0;
+    const bool art = (c->flags & F_ART_STRESS) != 0, xsph = (c->flags & F_XSPH) != 0;
     (void)p;
 #pragma omp parallel for schedule(dynamic, 64)
     for (i64 t = 0; t < nt; ++t) {
@@ -591,6 +598,7 @@ void orc_rhs(const orc_cfg *c, const orc_mat *mats, const orc_state *s, const do
 
         // ---- pair sums ----
         double drho = 0, dv[3] = {0, 0, 0}, du = 0, gv[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+        double xs[3] = {0, 0, 0}, Axs[3] = {0, 0, 0};
         double Adrho = 0, Adv[3] = {0, 0, 0}, Adu = 0, Agv[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
         for (i64 k = k0; k < k1; ++k) {
             i64 b = idx[k];
@@ -622,6 +630,21 @@ void orc_rhs(const orc_cfg *c, const orc_mat *mats, const orc_state *s, const do
                 Tm[al][be] = sigma[6 * a + IX[al][be]] / (rho_a * rho_a) + sigma[6 * b + IX[al][be]] / (s->rho[b] * s->rho[b]);
                 if (al == be) Tm[al][be] -= Pi;
             }
+            if (art) {                                                   // eqs. 35-38
+                double f = orc_W(D, r, H) / orc_W(D, c->as_mpd, H);      // eq. 38
+                double fn = std::pow(f, c->as_n);
+                for (int al = 0; al < D; ++al) for (int be = 0; be < D; ++be) {
+                    double sa = sigma[6 * a + IX[al][be]] / (rho_a * rho_a);
+                    double sb = sigma[6 * b + IX[al][be]] / (s->rho[b] * s->rho[b]);
+                    double za = (sa > 0.0) ? -c->as_eps * sa : 0.0;      // eq. 37: tension only (U25)
+                    double zb = (sb > 0.0) ? -c->as_eps * sb : 0.0;
+                    Tm[al][be] += (za + zb) * fn;                        // eqs. 35-36
+                }
+            }
+            if (xsph) {                                                  // eq. 40 (U26)
+                double wgt = c->xsph * 2.0 * s->m[b] / (rho_a + s->rho[b]) * orc_W(D, r, H);
+                for (int al = 0; al < D; ++al) { xs[al] += wgt * (-dvv[al]); Axs[al] += std::fabs(wgt * dvv[al]); }
+            }
             double e = 0.0;
             for (int al = 0; al < D; ++al) {
                 double f = 0.0;
@@ -642,6 +665,7 @@ void orc_rhs(const orc_cfg *c, const orc_mat *mats, const orc_state *s, const do
         drho = rho_a * drho;  Adrho = std::fabs(rho_a) * Adrho;
         o->drho[t] = drho; o->du[t] = du; o->A_drho[t] = Adrho; o->A_du[t] = Adu;
         for (int al = 0; al < 3; ++al) { o->dv[al][t] = dv[al]; o->A_dv[al][t] = Adv[al]; }
+        for (int al = 0; al < 3; ++al) { o->dxs[al][t] = xs[al]; o->A_dxs[al][t] = Axs[al]; }
         for (int al = 0; al < 3; ++al) for (int be = 0; be < 3; ++be) {
             o->gradv[3 * al + be][t] = gv[al][be]; o->A_gradv[3 * al + be][t] = Agv[al][be];
             o->C[3 * al + be][t] = C[al][be];

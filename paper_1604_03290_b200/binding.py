@@ -18,6 +18,7 @@ SPH_OK = 0
 SPH_ERR_ARG, SPH_ERR_STATE, SPH_ERR_WORKSPACE = -1, -2, -3
 SPH_ERR_NEIGHBOUR_OVERFLOW, SPH_ERR_TREE_DEPTH, SPH_ERR_CUDA = -4, -5, -6
 SPH_F_SOLID, SPH_F_PLASTIC, SPH_F_DAMAGE, SPH_F_GRAVITY, SPH_F_VARIABLE_H, SPH_F_DENSITY_SUM = 1, 2, 4, 8, 16, 32
+SPH_F_ART_STRESS, SPH_F_XSPH = 64, 128
 
 EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sph_build_tree",
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
@@ -38,7 +39,8 @@ class Config(C.Structure):
     _fields_ = [("dim", C.c_int32), ("flags", C.c_int32), ("n_materials", C.c_int32), ("morton_bits", C.c_int32),
                 ("max_neighbours", C.c_int32), ("n_des", C.c_int32), ("h_iters", C.c_int32), ("reserved", C.c_int32),
                 ("n", C.c_int64), ("n_flaws", C.c_int64), ("theta", C.c_double), ("G", C.c_double),
-                ("eps_soft", C.c_double), ("av_alpha", C.c_double), ("av_beta", C.c_double), ("av_eps", C.c_double)]
+                ("eps_soft", C.c_double), ("av_alpha", C.c_double), ("av_beta", C.c_double), ("av_eps", C.c_double),
+                ("as_eps", C.c_double), ("as_n", C.c_double), ("as_mpd", C.c_double), ("xsph", C.c_double)]
 
 
 class StateIn(C.Structure):
@@ -49,14 +51,15 @@ class StateIn(C.Structure):
 class StateOut(C.Structure):
     _fields_ = [("x", _vp * 3), ("v", _vp * 3), ("rho", _vp), ("u", _vp), ("S", _vp * 6), ("dmg", _vp), ("h", _vp),
                 ("drho", _vp), ("dv", _vp * 3), ("du", _vp), ("dS", _vp * 6), ("ddmg", _vp), ("ag", _vp * 3),
-                ("p", _vp), ("cs", _vp), ("strain", _vp), ("n_act", _vp), ("n_act_new", _vp), ("nb_count", _vp)]
+                ("p", _vp), ("cs", _vp), ("strain", _vp), ("n_act", _vp), ("n_act_new", _vp), ("nb_count", _vp),
+                ("dxs", _vp * 3)]
 
 
 _OUT_SHAPES = dict(x=3, v=3, rho=0, u=0, S=6, dmg=0, h=0, drho=0, dv=3, du=0, dS=6, ddmg=0, ag=3, p=0, cs=0,
-                   strain=0, n_act=0, n_act_new=0, nb_count=0)
+                   strain=0, n_act=0, n_act_new=0, nb_count=0, dxs=3)
 _OUT_INT = ("n_act", "n_act_new", "nb_count")
 STATE_FIELDS = ("x", "v", "rho", "u", "S", "dmg", "h", "n_act")
-RATE_FIELDS = ("drho", "dv", "du", "dS", "ddmg", "ag", "p", "cs", "strain", "n_act_new", "nb_count")
+RATE_FIELDS = ("drho", "dv", "du", "dS", "ddmg", "ag", "p", "cs", "strain", "n_act_new", "nb_count", "dxs")
 
 _lib = None
 
@@ -107,10 +110,12 @@ def load_library():
 
 
 def make_config(dim, n, flags, n_materials=1, morton_bits=21, max_neighbours=128, n_des=50, h_iters=0,
-                n_flaws=0, theta=0.5, G=0.0, eps_soft=0.0, av_alpha=1.0, av_beta=0.0, av_eps=0.01):
+                n_flaws=0, theta=0.5, G=0.0, eps_soft=0.0, av_alpha=1.0, av_beta=0.0, av_eps=0.01,
+                as_eps=0.2, as_n=4.0, as_mpd=1.0, xsph=0.5):
     return Config(dim=dim, flags=flags, n_materials=n_materials, morton_bits=morton_bits,
                   max_neighbours=max_neighbours, n_des=n_des, h_iters=h_iters, reserved=0, n=n, n_flaws=n_flaws,
-                  theta=theta, G=G, eps_soft=eps_soft, av_alpha=av_alpha, av_beta=av_beta, av_eps=av_eps)
+                  theta=theta, G=G, eps_soft=eps_soft, av_alpha=av_alpha, av_beta=av_beta, av_eps=av_eps,
+                  as_eps=as_eps, as_n=as_n, as_mpd=as_mpd, xsph=xsph)
 
 
 def make_materials(materials):
@@ -126,7 +131,7 @@ def config_of(w, h_iters=None, max_neighbours=None, morton_bits=21):
     cfg = make_config(w.dim, w.n, w.flags, len(w.materials), morton_bits,
                       w.max_neighbours if max_neighbours is None else max_neighbours, w.n_des,
                       w.h_iters if h_iters is None else h_iters, int(w.flaw_eps.size), w.theta, w.G, w.eps_soft,
-                      w.av_alpha, w.av_beta, w.av_eps)
+                      w.av_alpha, w.av_beta, w.av_eps, w.as_eps, w.as_n, w.as_mpd, w.xsph)
     return cfg, make_materials(w.materials)
 
 

@@ -39,6 +39,8 @@ bool cfg_ok(const sph_config *c) {
     if (c->n_flaws < 0) return false;
     if ((c->flags & SPH_F_GRAVITY) && !(c->theta >= 0.0 && c->theta * c->theta * c->dim < 1.0)) return false;
     if ((c->flags & SPH_F_VARIABLE_H) && c->h_iters > 0 && c->n_des < 1) return false;
+    if ((c->flags & SPH_F_ART_STRESS) && !(c->as_mpd > 0.0 && c->as_n > 0.0 && c->as_eps >= 0.0)) return false;
+    if ((c->flags & SPH_F_XSPH) && !(c->xsph >= 0.0 && c->xsph <= 1.0)) return false;
     return true;
 }
 
@@ -99,6 +101,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     for (int a = 0; a < 3; ++a) { z.dv[a] = b.take<double>(n); z.ag[a] = b.take<double>(n); }
     for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(n);
     z.n_act_new = b.take<int>(n);
+    for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? n : 1);
     z.stage = b.take<double>(n);
     z.stage_i = b.take<int>(n);
     Mats *md = b.take<Mats>(1);
@@ -179,7 +182,8 @@ __global__ void k_fill_d(double *dst, double v, size_t n) {
 }
 
 // A12, PAPER.md:388-394 (eqs. 52-53): q <- q0 + c * f, f = rates of the last evaluation (sorted
-// order, scattered through perm), dx/dt = v of the evaluated state (eq. 39 without XSPH).
+// order, scattered through perm), dx/dt = v of the evaluated state (eq. 39), plus the XSPH term of
+// eq. 40 with SPH_F_XSPH.
 // Every product and sum is rounded separately (reading O6).  After the update: dmg clamped to
 // [0, (n_act/n_tot)^(1/3)] (eq. 47), S <- f_Y S (eq. 16); n_act committed only when commit != 0.
 __global__ void k_update(Dev d, const sph_material *mats, double c, int commit) {
@@ -191,7 +195,8 @@ __global__ void k_update(Dev d, const sph_material *mats, double c, int commit) 
     const int D = d.D;
     for (int a = 0; a < 3; ++a) {
         if (a < D) {
-            const double vel = d.v[a][o];
+            double vel = d.v[a][o];
+            if (d.flags & SPH_F_XSPH) vel = __dadd_rn(vel, d.dxs[a][i]);      // eq. 40
             d.x[a][o] = __dadd_rn(q0[(size_t)a * n + o], __dmul_rn(c, vel));
             d.v[a][o] = __dadd_rn(q0[(size_t)(3 + a) * n + o], __dmul_rn(c, __dadd_rn(d.dv[a][i], d.ag[a][i])));
         } else {
@@ -268,6 +273,7 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     d.G = cfg->G;
     d.eps2 = cfg->eps_soft * cfg->eps_soft;
     d.av_alpha = cfg->av_alpha; d.av_beta = cfg->av_beta; d.av_eps = cfg->av_eps;
+    d.as_eps = cfg->as_eps; d.as_n = cfg->as_n; d.as_mpd = cfg->as_mpd; d.xsph = cfg->xsph;
     memset(&c->mats, 0, sizeof(c->mats));
     for (int k = 0; k < cfg->n_materials; ++k) c->mats.m[k] = materials[k];
     cudaMemcpyAsync(e->mats_dev, &c->mats, sizeof(Mats), cudaMemcpyHostToDevice, c->stream);
@@ -455,7 +461,7 @@ int sph_download(sph_ctx *ctx, const sph_state_out *o, int dst_is_device) {
     plain(o->n_act, d.n_act, (size_t)n * 4);
     const bool want_rates = o->drho || o->dv[0] || o->dv[1] || o->dv[2] || o->du || o->ddmg || o->ag[0] || o->ag[1] ||
                             o->ag[2] || o->p || o->cs || o->strain || o->n_act_new || o->nb_count || o->dS[0] ||
-                            o->dS[1] || o->dS[2] || o->dS[3] || o->dS[4] || o->dS[5];
+                            o->dS[1] || o->dS[2] || o->dS[3] || o->dS[4] || o->dS[5] || o->dxs[0] || o->dxs[1] || o->dxs[2];
     if (want_rates && !ctx->have_rates) return fail(ctx, SPH_ERR_STATE, "sph_download of rates before an evaluation");
     const int gb = sph_ceil_div(n, 256);
     auto unsort_d = [&](double *dst, const double *src, bool present) {
@@ -494,6 +500,7 @@ int sph_download(sph_ctx *ctx, const sph_state_out *o, int dst_is_device) {
     const bool solid = sph && (d.flags & SPH_F_SOLID), dam = sph && (d.flags & SPH_F_DAMAGE);
     unsort_d(o->drho, d.drho, sph); unsort_d(o->du, d.du, sph);
     for (int a = 0; a < 3; ++a) { unsort_d(o->dv[a], d.dv[a], sph); unsort_d(o->ag[a], d.ag[a], grav); }
+    for (int a = 0; a < 3; ++a) unsort_d(o->dxs[a], d.dxs[a], sph && (d.flags & SPH_F_XSPH));
     for (int k = 0; k < 6; ++k) unsort_d(o->dS[k], d.dS[k], solid);
     unsort_d(o->ddmg, d.ddmg, dam); unsort_d(o->strain, d.strain, dam);
     unsort_d(o->p, d.p, sph); unsort_d(o->cs, d.cs, sph);

@@ -199,7 +199,8 @@ __device__ __forceinline__ void cp_async_wait1() { asm volatile("cp.async.wait_g
 // memory by the whole warp -- 8 lanes fetch one record as 8 x 16 B, so a warp-wide copy touches 4
 // cache lines instead of 32 -- with cp.async one round ahead of the arithmetic; then every lane
 // reads ITS partner's record from shared memory (144-byte stride: conflict-free).
-template <int D, bool SOLID, bool VARH>
+// EXTRA: artificial stress (eqs. 35-38, reading U25) and/or the XSPH sum (eq. 40, reading U26).
+template <int D, bool SOLID, bool VARH, bool EXTRA>
 __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_material *mats) {
     constexpr int NS = (D == 3) ? 6 : 3;                 // independent stress components
     constexpr int SI[6] = {0, 1, (D == 3) ? 2 : 3, 3, 4, 5};   // 2-D: xx xy yy -> 0 1 3
@@ -233,6 +234,12 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
     double drho = 0.0, du = 0.0, dv[3] = {0, 0, 0};
     double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
     double N[6] = {0, 0, 0, 0, 0, 0};                     // symmetric moment matrix xx xy xz yy yz zz
+    double xs[3] = {0, 0, 0};                             // XSPH sum
+    const bool art = EXTRA && (d.flags & SPH_F_ART_STRESS), xsph = EXTRA && (d.flags & SPH_F_XSPH);
+    // kernel shape w(q) = W h^D / s (eq. 25): 6q^3 - 6q^2 + 1 below q = 1/2, 2 (1 - q)^3 above
+    auto wshape = [](double q) { const double t = fmax(1.0 - q, 0.0); return (q < 0.5) ? fma(6.0 * q * q, q - 1.0, 1.0) : 2.0 * t * t * t; };
+    const double wnorm_i = KNorm<D>::s * ((D == 3) ? iHi * iHi * iHi : iHi * iHi);
+    const double wm_i = EXTRA ? wshape(d.as_mpd * iHi) : 1.0;
 
     // copy the records of partners `b` (one per lane) into buffer `buf`
     const int sub = lane & 7, row0 = lane >> 3;
@@ -295,6 +302,24 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
             }
             double T[NS];
             for (int k2 = 0; k2 < NS; ++k2) T[k2] = sa[k2] + sb6[SI[k2]];
+            if (EXTRA) {
+                const double wq = wshape(q);
+                if (art) {                                    // eqs. 35-38: repulsive stress in tension
+                    const double wm = VARH ? wshape(d.as_mpd * iH) : wm_i;
+                    const double fr = wq / wm;                // eq. 38
+                    const double fn = (d.as_n == 4.0) ? (fr * fr) * (fr * fr) : pow(fr, d.as_n);
+                    for (int k2 = 0; k2 < NS; ++k2) {
+                        const double s1 = sa[k2], s2 = sb6[SI[k2]];
+                        const double z = ((s1 > 0.0) ? s1 : 0.0) + ((s2 > 0.0) ? s2 : 0.0);   // eq. 37 (U25)
+                        T[k2] -= d.as_eps * z * fn;
+                    }
+                }
+                if (xsph) {                                   // eq. 40 (U26)
+                    const double wn = VARH ? KNorm<D>::s * ((D == 3) ? iH * iH * iH : iH * iH) : wnorm_i;
+                    const double wgt = d.xsph * 2.0 * mb / (rhoi + rhob) * (wn * wq);
+                    for (int a = 0; a < D; ++a) xs[a] -= wgt * dvv[a];
+                }
+            }
             double fv[3];
             if (D == 3) {
                 T[0] -= Pi; T[3] -= Pi; T[5] -= Pi;
@@ -307,7 +332,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
                 fv[1] = T[1] * gW[0] + T[2] * gW[1];
             }
             double e = 0.0;
-            for (int a = 0; a < D; ++a) { dv[a] += mb * fv[a]; e += fv[a] * dvv[a]; }   // eqs. 30/34
+            for (int a = 0; a < D; ++a) { dv[a] += mb * fv[a]; e += fv[a] * dvv[a]; }   // eqs. 30/34 (35 with artificial stress)
             du += mb * e;                                                             // eq. 31 (x -1/2 below)
             if (SOLID) {
                 for (int a = 0; a < D; ++a) {
@@ -326,6 +351,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
     d.drho[i] = rhoi * drho;
     d.du[i] = -0.5 * du;
     for (int a = 0; a < 3; ++a) d.dv[a][i] = (a < D) ? dv[a] : 0.0;
+    if (xsph) for (int a = 0; a < 3; ++a) d.dxs[a][i] = (a < D) ? xs[a] : 0.0;
 
     const sph_material mt = mats[d.smat[i]];
     double St[6] = {0, 0, 0, 0, 0, 0};
@@ -432,13 +458,16 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
         ctx->launches += 1;
     }
     StageTimer tm(ctx, SPH_T_PAIRS);
+    const bool extra = (d.flags & (SPH_F_ART_STRESS | SPH_F_XSPH)) != 0;
+#define SPH_PAIRS(S, V, E) k_pairs<D, S, V, E><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats)
     if (solid) {
-        if (varh) k_pairs<D, true, true><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
-        else k_pairs<D, true, false><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
+        if (varh) { if (extra) SPH_PAIRS(true, true, true); else SPH_PAIRS(true, true, false); }
+        else { if (extra) SPH_PAIRS(true, false, true); else SPH_PAIRS(true, false, false); }
     } else {
-        if (varh) k_pairs<D, false, true><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
-        else k_pairs<D, false, false><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats);
+        if (varh) { if (extra) SPH_PAIRS(false, true, true); else SPH_PAIRS(false, true, false); }
+        else { if (extra) SPH_PAIRS(false, false, true); else SPH_PAIRS(false, false, false); }
     }
+#undef SPH_PAIRS
     ctx->launches += 1;
 }
 

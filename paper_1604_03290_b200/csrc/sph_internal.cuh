@@ -72,6 +72,7 @@ struct Dev {
     int n;
     int n_des;
     double theta2, G, eps2, av_alpha, av_beta, av_eps;
+    double as_eps, as_n, as_mpd, xsph;
     // ---- master state, original order ----
     double *x[3], *v[3], *m, *rho, *u, *S[6], *dmg, *h;
     int *mat, *n_act;
@@ -117,6 +118,7 @@ struct Dev {
     double *prec;               // PR_REC doubles per particle: x3 v3 rho m/rho cs h sigma/rho^2 (6)
     // ---- rates, sorted order ----
     double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *strain;
+    double *dxs[3];             // XSPH term of eq. 40 (only with SPH_F_XSPH)
     int *n_act_new;
     // ---- staging ----
     double *stage;              // n doubles, for unsorting downloads

@@ -35,6 +35,8 @@ F_DAMAGE = 4
 F_GRAVITY = 8
 F_VARIABLE_H = 16
 F_DENSITY_SUM = 32
+F_ART_STRESS = 64      # artificial stress, PAPER.md:284-302 (eqs. 35-38)
+F_XSPH = 128           # XSPH velocity smoothing, PAPER.md:311 (eq. 40)
 
 EOS_IDEAL_GAS = 0
 EOS_MURNAGHAN = 1
@@ -88,6 +90,10 @@ class Workload:
     av_alpha: float = 1.0
     av_beta: float = 0.0
     av_eps: float = 0.01
+    as_eps: float = 0.2    # artificial stress factor, exponent n and mean particle distance (eqs. 37-38)
+    as_n: float = 4.0
+    as_mpd: float = 1.0
+    xsph: float = 0.5      # XSPH factor of eq. 40
     n_des: int = 50
     h_iters: int = 0
     dt: float = 1e-3
@@ -260,6 +266,16 @@ def c1_rubber_rings(seed=1604, scale=1.0, twin=False):
     return w
 
 
+def c1x_rubber_rings_paper(seed=1604, scale=1.0, twin=False):
+    """C1 with the settings of the paper's own ring test: artificial stress
+    eps_s = 0.2, n = 4, dmpd = the lattice spacing, and XSPH with x_sph = 0.5."""
+    w = c1_rubber_rings(seed=seed, scale=scale, twin=twin)
+    w.name = w.name.replace("C1", "C1x")
+    w.flags |= F_ART_STRESS | F_XSPH
+    w.as_eps, w.as_n, w.as_mpd, w.xsph = 0.2, 4.0, w.meta["dx"], 0.5
+    return w
+
+
 # ----------------------------------------------------------------------------------------
 # C2: 3-D self-gravitating gas sphere, rho ~ 1/r (BASELINE.json configs[1])
 # ----------------------------------------------------------------------------------------
@@ -387,7 +403,7 @@ def c5_ceres_collision(seed=1608, scale=1.0, twin=False):
     return w
 
 
-CONFIGS = {"C1": c1_rubber_rings, "C2": c2_gas_sphere, "C3": c3_al_impact,
+CONFIGS = {"C1": c1_rubber_rings, "C1x": c1x_rubber_rings_paper, "C2": c2_gas_sphere, "C3": c3_al_impact,
            "C4": c4_basalt_impact, "C5": c5_ceres_collision}
 
 

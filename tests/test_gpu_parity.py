@@ -94,6 +94,10 @@ def check_rates(w, g, o, targets=None):
         assert_close("ag", g["ag"][:, t], o["ag"], o["A_ag"])
     if w.flags & orc.F_DENSITY_SUM:
         assert_close("rho", g["rho"][t], o["rho"][t], rel=1e-12)
+    if w.flags & orc.F_XSPH:
+        assert_close("dxs", g["dxs"][:, t], o["dxs"], o["A_dxs"])
+    else:
+        assert not g["dxs"].any()
     if w.flags & orc.F_DAMAGE:
         # strain = sigma_max / ((1 - d) E): the eigenvalue carries an error relative to |sigma|, not to itself
         tt = np.arange(w.n)[t]
@@ -114,9 +118,18 @@ def check_rates(w, g, o, targets=None):
         assert_close("ddmg", g["ddmg"][t][same], o["ddmg"][same], rel=1e-10)
 
 
+def _with_art(w):
+    w.flags |= sph_inputs.F_ART_STRESS | sph_inputs.F_XSPH
+    w.as_eps, w.as_n, w.as_mpd, w.xsph = 0.3, 3.0, (1.0 / w.n) ** (1.0 / w.dim), 0.5     # n != 4: the pow() path
+    return w
+
+
 CASES = {
     "C1-twin": lambda: sph_inputs.make("C1", scale=0.25, twin=True),
     "C1-nominal": lambda: sph_inputs.make("C1", scale=0.25),
+    "C1x-twin": lambda: sph_inputs.make("C1x", scale=0.25, twin=True),      # artificial stress + XSPH
+    "blob3d-art": lambda: _with_art(sph_inputs.random_blob(2200, dim=3, seed=6, duplicates=3)),
+    "blob3d-varh-art": lambda: _with_art(sph_inputs.random_blob(1800, dim=3, seed=7, variable_h=True)),
     "C2-twin": lambda: sph_inputs.c2_gas_sphere(n=3000, twin=True),
     "C3-twin": lambda: sph_inputs.make("C3", scale=0.006, twin=True),
     "C4-twin": lambda: sph_inputs.make("C4", scale=0.002, twin=True),
@@ -207,7 +220,7 @@ def test_device_resident_upload_and_download(P):
         assert np.array_equal(gd[k].cpu().numpy(), gh[k]), k
 
 
-@pytest.mark.parametrize("name", ["C1-twin", "C4-twin", "C2-twin"])
+@pytest.mark.parametrize("name", ["C1-twin", "C4-twin", "C2-twin", "C1x-twin"])
 def test_step_parity(P, name):
     """sph_step = two complete evaluations + two updates (eqs. 52-53).  Per-evaluation parity is the
     contract; the trajectory after a step is compared with a looser bound (rates enter multiplied by dt)."""

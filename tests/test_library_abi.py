@@ -34,11 +34,11 @@ def test_every_declared_symbol_is_exported(lib):
 
 
 def test_struct_layouts_match_header():
-    # sizes implied by include/sph.h (LP64): material 2*int32 + 15 doubles; config 8*int32 + 2*int64 + 6 doubles
+    # sizes implied by include/sph.h (LP64): material 2*int32 + 15 doubles; config 8*int32 + 2*int64 + 10 doubles
     assert C.sizeof(P.Material) == 8 + 15 * 8
-    assert C.sizeof(P.Config) == 32 + 16 + 48
+    assert C.sizeof(P.Config) == 32 + 16 + 80
     assert C.sizeof(P.binding.StateIn) == 8 * (3 + 3 + 3 + 6 + 2 + 2 + 2)
-    assert C.sizeof(P.binding.StateOut) == 8 * (3 + 3 + 2 + 6 + 2 + 1 + 3 + 1 + 6 + 1 + 3 + 3 + 3)
+    assert C.sizeof(P.binding.StateOut) == 8 * (3 + 3 + 2 + 6 + 2 + 1 + 3 + 1 + 6 + 1 + 3 + 3 + 3 + 3)
 
 
 def test_workspace_sizing_and_config_validation(lib):
