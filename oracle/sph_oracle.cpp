@@ -18,7 +18,9 @@
 // Parity pins: every function here is pinned by tests/test_oracle_*.py (closed forms,
 // invariants, brute force) EXCEPT the two readings the paper cannot pin:
 //   * crack growth speed c_g and the length R_s in eqs. 24/46 (U16): "parity unpinned"
-//     by the paper (pinned only by dimensional analysis and the hand-computed formula).
+//     by the paper (pinned only by dimensional analysis and the hand-computed formula);
+//   * the per-component tension criterion of the artificial stress, eq. 37 (U25): "parity
+//     unpinned" by the paper (pinned by a two-particle closed form and the conservation identities).
 // =====================================================================================
 #include <algorithm>
 #include <cmath>

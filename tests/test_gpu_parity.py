@@ -315,3 +315,31 @@ def test_error_paths(P):
     h = C.c_void_p()
     assert L.sph_create(C.byref(cfg), mats, C.c_void_p(buf.data_ptr()), 1 << 20, None, C.byref(h)) == P.SPH_ERR_WORKSPACE
     assert L.sph_create(C.byref(cfg), mats, C.c_void_p(buf.data_ptr() + 8), 1 << 40, None, C.byref(h)) == P.SPH_ERR_WORKSPACE
+
+
+def test_gravity_theta_zero_is_direct_sum_and_deep_stack(P):
+    """theta = 0 opens every cell: the walk degenerates to the direct sum and the
+    shared-memory stack of the gravity kernel sees its deepest load."""
+    w = sph_inputs.random_blob(6000, dim=3, seed=12, duplicates=40)
+    w.theta = 0.0
+    ctx = make_ctx(P, w)
+    ctx.build_tree()
+    ctx.gravity()
+    ctx.sync()
+    g = ctx.download(("ag",))["ag"]
+    ag, _ = orc.gravity_direct(w)
+    A = np.abs(ag).sum(axis=0) + 1e-300
+    scale = np.abs(ag).max()
+    assert np.all(np.abs(g - ag) <= 1e-10 * np.abs(ag) + 1e-12 * scale)
+    c = ctx.get_counters()
+    assert c["n_visit"] > 0
+    ctx.close()
+    # 2-D as well (quadtree: four children per cell)
+    w = sph_inputs.random_blob(3000, dim=2, seed=13)
+    w.theta = 0.0
+    ctx = make_ctx(P, w)
+    ctx.build_tree(); ctx.gravity(); ctx.sync()
+    g = ctx.download(("ag",))["ag"]
+    ag, _ = orc.gravity_direct(w)
+    assert np.all(np.abs(g - ag) <= 1e-10 * np.abs(ag) + 1e-12 * np.abs(ag).max())
+    ctx.close()
