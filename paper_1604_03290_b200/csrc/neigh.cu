@@ -22,7 +22,7 @@
 // reads them fully coalesced; within a list partners come in ascending Morton order.
 #include "sph_internal.cuh"
 
-#define NB_WARPS 8
+#define NB_WARPS 2
 
 // ------------------------------------------------------------------------------------------
 // search stream layout

@@ -184,7 +184,7 @@ __device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02
     }
 }
 
-#define PR_WARPS 4
+#define PR_WARPS 1
 #define PR_STRIDE 18            // doubles between staged records (144 B): 16-byte reads by lane are conflict-free
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
