@@ -148,6 +148,15 @@ int sph_evaluate(sph_ctx *ctx);
 /* A12: predictor-corrector step (eqs. 52-53): two complete evaluations and two updates. */
 int sph_step(sph_ctx *ctx, double dt);
 
+/* Upper limits of the next time step from the rates of the LAST complete evaluation:
+ *   out[0] = min_a 0.2 h_a / |dv_a/dt|       (eq. 54; the acceleration includes self-gravity)
+ *   out[1] = min_a 0.7 h_a / c_s,a           (eq. 55, Courant)
+ *   out[2] = min_a,q 0.7 |q_a| / |dq_a/dt|   (eq. 57) over q = rho (not with SPH_F_DENSITY_SUM), u, the
+ *            components of S (SPH_F_SOLID) and dmg (SPH_F_DAMAGE); entries with q = 0 or dq/dt = 0 are skipped
+ *   out[3] = the smallest of the three       (eq. 56 with eq. 57)
+ * A limit that no particle sets is +infinity.  out: HOST double[4].  Synchronises. */
+int sph_timestep(sph_ctx *ctx, double *out);
+
 /* Copy state and/or the rates of the last evaluation out, original order.
  * dst_is_device: 1 = DEVICE buffers (asynchronous), 0 = HOST buffers (synchronises). */
 int sph_download(sph_ctx *ctx, const sph_state_out *dst, int dst_is_device);

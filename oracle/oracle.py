@@ -358,6 +358,36 @@ def evaluate(w, mode="brute", targets=None, h_iters=None):
     return out
 
 
+def timestep(w, e):
+    """Time-step limits of PAPER.md:396-414 from the workload state `w` and the rates `e` of one
+    evaluation of ALL particles (evaluate(w, ...)):  eq. 54 (0.2 h/|dv/dt|, gravity included), eq. 55
+    (0.7 h/c_s), eq. 57 (0.7 |q|/|dq/dt| over rho, u, the components of S and dmg; entries with q = 0
+    or dq/dt = 0 are skipped: reading U28) and their minimum (eq. 56).  +inf where nobody sets a limit."""
+    D, inf = w.dim, float("inf")
+    h = e["h"]
+    out = {}
+    acc = np.sqrt(((e["dv"] + e["ag"])[:D] ** 2).sum(axis=0))
+    out["acceleration"] = min([0.2 * h[a] / acc[a] for a in range(w.n) if acc[a] > 0.0], default=inf)
+    cs = e["cs"]
+    out["courant"] = min([0.7 * h[a] / cs[a] for a in range(w.n) if cs[a] > 0.0], default=inf)
+    pairs = [(w.u, e["du"])]
+    if not (w.flags & F_DENSITY_SUM):
+        pairs.append((e["rho"], e["drho"]))
+    if w.flags & F_SOLID:
+        comps = (0, 1, 3) if D == 2 else range(6)
+        pairs += [(w.S[k], e["dS"][k]) for k in comps]
+    if w.flags & F_DAMAGE:
+        pairs.append((w.dmg, e["ddmg"]))
+    lim = inf
+    for q, dq in pairs:
+        for a in range(w.n):
+            if q[a] != 0.0 and dq[a] != 0.0:
+                lim = min(lim, 0.7 * abs(q[a]) / abs(dq[a]))
+    out["change"] = lim
+    out["dt_max"] = min(out.values())
+    return out
+
+
 def _limit(w):
     """S <- f_Y S after an update (eq. 16); dmg clamp (eq. 47)."""
     D = w.dim

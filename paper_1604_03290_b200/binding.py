@@ -24,7 +24,7 @@ EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sp
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
-           "sph_timing_name", "sph_get_counters", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+           "sph_timing_name", "sph_get_counters", "sph_timestep", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
 SPH_T_COUNT = 11
 
 _vp = C.c_void_p
@@ -103,6 +103,7 @@ def load_library():
     L.sph_timing_name.restype = C.c_char_p
     L.sph_timing_name.argtypes = [C.c_int]
     L.sph_get_counters.argtypes = [_vp, _vp]
+    L.sph_timestep.argtypes = [_vp, _vp]
     L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
     L.sph_measure_copy_bw.argtypes = [_vp, _vp, _vp, C.c_size_t, C.POINTER(C.c_double)]
     _lib = L
@@ -306,6 +307,12 @@ class Context:
         self._check(L.sph_timing_read(self.handle, ms.ctypes.data, ln.ctypes.data))
         return {L.sph_timing_name(k).decode(): (float(ms[k]), int(ln[k])) for k in range(SPH_T_COUNT)}
 
+    def timestep(self):
+        """sph_timestep: dict of the limits of eqs. 54, 55, 57 and their minimum (eq. 56)."""
+        out = np.zeros(4)
+        self._check(load_library().sph_timestep(self.handle, out.ctypes.data))
+        return dict(acceleration=float(out[0]), courant=float(out[1]), change=float(out[2]), dt_max=float(out[3]))
+
     def get_counters(self):
         out = np.zeros(4, np.int64)
         self._check(load_library().sph_get_counters(self.handle, out.ctypes.data))
@@ -359,6 +366,10 @@ def sph_step(ctx, dt):
 
 def sph_download(ctx, fields=STATE_FIELDS + RATE_FIELDS, device=False, out=None):
     return ctx.download(fields, device, out)
+
+
+def sph_timestep(ctx):
+    return ctx.timestep()
 
 
 def sph_sync(ctx):

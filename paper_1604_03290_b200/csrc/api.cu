@@ -238,6 +238,49 @@ __global__ void k_update(Dev d, const sph_material *mats, double c, int commit) 
     }
 }
 
+// PAPER.md:396-414 (eqs. 54-57): time-step limits, one min-reduction over the particles (sorted order).
+// Positive doubles order like their bit patterns, so the block minima are combined with atomicMin on u64.
+__global__ void k_dtlim_init(Dev d) {
+    if (threadIdx.x < 3) d.status->dtlim[threadIdx.x] = 0x7ff0000000000000ull;
+}
+__global__ void __launch_bounds__(256) k_dtlim(Dev d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const double inf = __longlong_as_double(0x7ff0000000000000ll);
+    double t[3] = {inf, inf, inf};
+    if (i < d.n) {
+        const double h = d.sh[i];
+        double a2 = 0.0;
+        for (int a = 0; a < d.D; ++a) { const double acc = d.dv[a][i] + d.ag[a][i]; a2 += acc * acc; }
+        if (a2 > 0.0) t[0] = 0.2 * h / sqrt(a2);                       // eq. 54
+        const double cs = d.cs[i];
+        if (cs > 0.0) t[1] = 0.7 * h / cs;                              // eq. 55
+        auto lim = [&](double q, double dq) {                          // eq. 57
+            if (q != 0.0 && dq != 0.0) t[2] = fmin(t[2], 0.7 * fabs(q) / fabs(dq));
+        };
+        if (!(d.flags & SPH_F_DENSITY_SUM)) lim(d.srho[i], d.drho[i]);
+        lim(d.su[i], d.du[i]);
+        if (d.flags & SPH_F_SOLID) {
+            for (int k = 0; k < 6; ++k) {
+                if (d.D == 2 && (k == 2 || k == 4 || k == 5)) continue;
+                lim(d.sS[k][i], d.dS[k][i]);
+            }
+        }
+        if (d.flags & SPH_F_DAMAGE) lim(d.sdmg[i], d.ddmg[i]);
+    }
+    __shared__ double s_min[3][8];
+    for (int k = 0; k < 3; ++k) {
+        double v = t[k];
+        for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+        if ((threadIdx.x & 31) == 0) s_min[k][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double v = s_min[threadIdx.x][0];
+        for (int w = 1; w < 8; ++w) v = fmin(v, s_min[threadIdx.x][w]);
+        atomicMin(&d.status->dtlim[threadIdx.x], (u64)__double_as_longlong(v));
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // C ABI
 // ------------------------------------------------------------------------------------------------
@@ -339,6 +382,22 @@ int sph_get_counters(sph_ctx *ctx, int64_t *out) {
     cudaStreamSynchronize(ctx->stream);
     out[0] = st.n_nodes; out[1] = (int64_t)st.n_pairs; out[2] = (int64_t)st.n_inter; out[3] = (int64_t)st.n_visit;
     return check_cuda(ctx, "sph_get_counters");
+}
+
+int sph_timestep(sph_ctx *ctx, double *out) {
+    if (!ctx || !out) return SPH_ERR_ARG;
+    if ((ctx->have_rates & 1) == 0 || ((ctx->d.flags & SPH_F_GRAVITY) && (ctx->have_rates & 2) == 0))
+        return fail(ctx, SPH_ERR_STATE, "sph_timestep before a complete evaluation");
+    Dev &d = ctx->d;
+    k_dtlim_init<<<1, 32, 0, ctx->stream>>>(d);
+    k_dtlim<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
+    ctx->launches += 2;
+    DevStatus st;
+    cudaMemcpyAsync(&st, d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    for (int k = 0; k < 3; ++k) memcpy(&out[k], &st.dtlim[k], sizeof(double));
+    out[3] = std::min(out[0], std::min(out[1], out[2]));
+    return check_cuda(ctx, "sph_timestep");
 }
 
 int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {

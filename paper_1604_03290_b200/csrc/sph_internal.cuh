@@ -26,6 +26,7 @@ struct DevStatus {
     u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
     int n_items;        // records of the partner-search stream
     int pad;
+    u64 dtlim[3];       // bit patterns of the three time-step limits (positive doubles order like integers)
 };
 
 // Root cube of the last build (device).

@@ -343,3 +343,19 @@ def test_gravity_theta_zero_is_direct_sum_and_deep_stack(P):
     ag, _ = orc.gravity_direct(w)
     assert np.all(np.abs(g - ag) <= 1e-10 * np.abs(ag) + 1e-12 * np.abs(ag).max())
     ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C5-twin", "C2-twin", "C1x-twin"])
+def test_timestep_limits(P, name):
+    """sph_timestep (eqs. 54-57) against the oracle's limits from its own rates."""
+    w = CASES[name]()
+    ctx = make_ctx(P, w, h_iters=0)
+    with pytest.raises(P.SphError):
+        ctx.timestep()                                   # no evaluation yet
+    ctx.evaluate()
+    t = ctx.timestep()
+    o = orc.evaluate(w, mode="brute", h_iters=0)
+    want = orc.timestep(w, o)
+    for k in ("acceleration", "courant", "change", "dt_max"):
+        assert t[k] == pytest.approx(want[k], rel=1e-9), k
+    ctx.close()

@@ -107,3 +107,30 @@ def test_artificial_stress_keeps_momentum_and_energy_identities(D):
     # continuity, velocity gradient and dS/dt do not see the artificial stress
     for k in ("drho", "dS", "gradv"):
         assert np.array_equal(e[k], e0[k]), k
+
+
+# ------------------------------------------------------------------ time-step limits
+def test_timestep_limits_hand_values_and_scaling():
+    """eqs. 54-57 on hand-made rates: the planted particle sets each limit; h scales eqs. 54-55."""
+    w = si.random_blob(50, 3, 2, gravity=False, damage=False)
+    n = w.n
+    e = dict(h=w.h.copy(), dv=np.full((3, n), 1e-3), ag=np.zeros((3, n)), cs=np.full(n, 2.0), rho=w.rho.copy(),
+             drho=np.zeros(n), du=np.zeros(n), dS=np.zeros((6, n)), ddmg=np.zeros(n))
+    e["dv"][:, 7] = (3.0, 4.0, 12.0)                       # |dv/dt| = 13
+    e["cs"][11] = 50.0
+    e["du"][5] = -4.0 * abs(w.u[5])                         # 0.7 |u|/|du/dt| = 0.175
+    t = orc.timestep(w, e)
+    assert t["acceleration"] == pytest.approx(0.2 * w.h[7] / 13.0, rel=1e-15)
+    assert t["courant"] == pytest.approx(0.7 * w.h[11] / 50.0, rel=1e-15)
+    assert t["change"] == pytest.approx(0.175, rel=1e-14)
+    assert t["dt_max"] == min(t["acceleration"], t["courant"], t["change"])
+    e2 = dict(e); e2["h"] = 2.0 * e["h"]
+    t2 = orc.timestep(w, e2)
+    assert t2["acceleration"] == pytest.approx(2.0 * t["acceleration"]) and t2["courant"] == pytest.approx(2.0 * t["courant"])
+    assert t2["change"] == t["change"]
+    # gravity enters eq. 54
+    e3 = dict(e); e3["ag"] = -e["dv"]
+    assert orc.timestep(w, e3)["acceleration"] == float("inf")
+    # nobody limits: +inf
+    e4 = dict(e); e4["du"] = np.zeros(n)
+    assert orc.timestep(w, e4)["change"] == float("inf")
