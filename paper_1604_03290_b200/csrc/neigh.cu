@@ -102,8 +102,8 @@ __global__ void k_emit_items(Dev d) {
                 const u64 sc = d.bscan[s0], m0 = d.bmark[s0];
                 const int pos = (int)(sc & 0xffffffffu) + (int)(sc >> 32) + (int)(m0 >> 32);
                 SearchItem it;
-                for (int a = 0; a < 3; ++a) { it.bmin[a] = mn[a]; it.bmax[a] = mx[a]; }
-                it.hmax = hm; it.skip = -len; it.lo = s0;
+                for (int a = 0; a < 3; ++a) { it.bmin[a] = __double2float_rd(mn[a]); it.bmax[a] = __double2float_ru(mx[a]); }
+                it.hmax = __double2float_ru(hm); it.pad = 0.f; it.skip = -len; it.lo = s0; it.pad2[0] = it.pad2[1] = 0;
                 d.items[pos] = it;
             }
         }
@@ -115,8 +115,8 @@ __global__ void k_emit_items(Dev d) {
             while (t - 1 - k >= 0 && d.nlo[t - 1 - k] == lo) ++k;     // ancestors sharing lo precede it
             const u64 sl = d.bscan[lo], sh_ = d.bscan[hi];
             SearchItem it;
-            for (int a = 0; a < 3; ++a) { it.bmin[a] = d.nbmin[a][t]; it.bmax[a] = d.nbmax[a][t]; }
-            it.hmax = d.nhmax[t];
+            for (int a = 0; a < 3; ++a) { it.bmin[a] = __double2float_rd(d.nbmin[a][t]); it.bmax[a] = __double2float_ru(d.nbmax[a][t]); }
+            it.hmax = __double2float_ru(d.nhmax[t]); it.pad = 0.f; it.pad2[0] = it.pad2[1] = 0;
             it.skip = (int)(sh_ & 0xffffffffu) + (int)(sh_ >> 32);
             it.lo = lo;
             d.items[(int)(sl & 0xffffffffu) + (int)(sl >> 32) + k] = it;
@@ -157,7 +157,10 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     const double xi = d.sx[0][ii], yi = d.sx[1][ii], zi = (D == 3) ? d.sx[2][ii] : 0.0;
     const double Hi = d.sh[ii];
     const double Hi2 = __dmul_rn(Hi, Hi);
-    const double slack = 1.0 + 1e-9;            // the pruning test must never cut a true partner
+    constexpr bool VH = VARH && !COUNT_ONLY;   // pair criterion (h_a + h_b)/2, eq. 72
+    const float xlo = __double2float_rd(xi), xhi = __double2float_ru(xi), ylo = __double2float_rd(yi), yhi = __double2float_ru(yi);
+    const float zlo = __double2float_rd(zi), zhi = __double2float_ru(zi);
+    const float Hf = __double2float_ru(Hi) * 1.000001f;      // the pruning test must never cut a true partner
 
     int cnt = 0;
     int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
@@ -168,15 +171,17 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     int next = valid ? 0 : 0x7fffffff;
     int cur = 0;
     while (cur < nitems) {
-        const double2 *rec = reinterpret_cast<const double2 *>(items + cur);
-        const double2 q0 = __ldg(rec), q1 = __ldg(rec + 1), q2 = __ldg(rec + 2), q3 = __ldg(rec + 3);
-        const double4 b0 = make_double4(q0.x, q0.y, q1.x, q1.y);      // bmin xyz, bmax x
-        const double4 b1 = make_double4(q2.x, q2.y, q3.x, q3.y);      // bmax yz, hmax, (skip, lo)
-        const int skip = __double2loint(b1.w), lo = __double2hiint(b1.w);
+        // pruning in FP32 with directed rounding: the boxes are rounded outward, the particle towards
+        // the box, the differences down and the reach up, so a box that a partner lies in is never cut
+        const float4 *rec = reinterpret_cast<const float4 *>(items + cur);
+        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);            // bmin xyz bmax x | bmax yz hmax pad
+        const int2 sl = __ldg(reinterpret_cast<const int2 *>(rec + 2));
+        const int skip = sl.x, lo = sl.y;
         const bool act = (next == cur);
-        const double reach = ((VARH && !COUNT_ONLY) ? 0.5 * (Hi + b1.z) : Hi) * slack;
-        bool ov = act && (b0.x - xi <= reach) && (xi - b0.w <= reach) && (b0.y - yi <= reach) && (yi - b1.x <= reach);
-        if (D == 3) ov = ov && (b0.z - zi <= reach) && (zi - b1.y <= reach);
+        const float reach = VH ? __fmul_ru(0.5f, __fadd_ru(Hf, r1.z)) * 1.000001f : Hf;
+        bool ov = act && (__fsub_rd(r0.x, xhi) <= reach) && (__fsub_rd(xlo, r0.w) <= reach) &&
+                  (__fsub_rd(r0.y, yhi) <= reach) && (__fsub_rd(ylo, r1.x) <= reach);
+        if (D == 3) ov = ov && (__fsub_rd(r0.z, zhi) <= reach) && (__fsub_rd(zlo, r1.y) <= reach);
         if (skip >= 0) {
             if (act) next = ov ? cur + 1 : skip;
         } else {

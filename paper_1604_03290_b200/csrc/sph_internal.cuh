@@ -44,9 +44,11 @@ struct DevRoot {
 #define PR_REC 16
 #define SPH_BUCKET 32
 struct __align__(16) SearchItem {
-    double bmin[3], bmax[3];    // tight bounding box of the particles below
-    double hmax;                // largest smoothing length below
+    float bmin[3], bmax[3];     // box of the particles below, rounded OUTWARD to FP32 (pruning only)
+    float hmax;                 // largest smoothing length below, rounded up
+    float pad;
     int skip, lo;
+    int pad2[2];
 };
 
 // Gravity records (gravity.cu): one per octree cell and per leaf, the children of a cell contiguous.
