@@ -71,7 +71,7 @@ __global__ void k_emit_items(Dev d) {
         d.status->n_items = (int)(tot & 0xffffffffu) + (int)(tot >> 32);
     }
     {   // buckets: the warp handles the bucket starts among its 32 positions one after the other,
-        // all lanes loading the (<= 32) members together (one thread per bucket with a serial loop
+        // all lanes loading the (<= SPH_BUCKET) members together (one thread per bucket with a serial loop
         // cost 0.5 ms on C5: profiles/r1d_c5.md)
         const unsigned FULL = 0xffffffffu;
         const int lane = threadIdx.x & 31, base = t - lane;
@@ -81,7 +81,7 @@ __global__ void k_emit_items(Dev d) {
             const int j = __ffs(starts) - 1;
             starts &= starts - 1;
             const int s0 = base + j;
-            const int q = s0 + 1 + lane;                       // a bucket has at most SPH_BUCKET = 32 members
+            const int q = s0 + 1 + lane;                       // a bucket has at most SPH_BUCKET <= 32 members
             const bool stop = (q >= n) || ((d.bmark[q] & 1ull) != 0ull);
             const int len = __ffs(__ballot_sync(FULL, stop));  // members: s0 .. s0 + len - 1
             const bool have = lane < len;
