@@ -419,10 +419,10 @@ def main():
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures under profiles/ (filled in per round; None = not captured yet).
 TRAFFIC_NCU = {
-    # profiles/r1d_c5.md: k_gravity<3,4,2,0> 0.317 GB read + 0.083 GB written per launch
-    ("C5", "gravity"): 399.9e6,
-    ("C5", "pairs"): 3147.8e6,
-    ("C5", "neighbours"): 2498.8e6,
+    # profiles/r1e_c5.md: k_gravity<3,4,2,0> 0.317 GB read + 0.084 GB written per launch
+    ("C5", "gravity"): 401.0e6,
+    ("C5", "pairs"): 3147.3e6,
+    ("C5", "neighbours"): 2919.0e6,
 }
 
 if __name__ == "__main__":
