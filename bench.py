@@ -146,7 +146,9 @@ def run_ours(args, rank, world):
     w = sph_inputs.make(args.workload, scale=args.scale, seed=sph_inputs_seed(args.workload) + rank)
     t_gen = time.time() - t_gen
     cfg, mats = P.config_of(w)
-    ctx = P.sph_create(cfg, mats, device=dev)
+    stream = torch.cuda.Stream(device=dev)     # a stream of our own: sph_step may capture it into a CUDA graph
+    torch.cuda.set_stream(stream)              # torch's events, fills and copies below go to the same stream
+    ctx = P.sph_create(cfg, mats, device=dev, stream=stream)
     ctx.upload_workload(w)
     ws_bytes = ctx.workspace_bytes
     small = ws_bytes < 4 * L2_BYTES       # working set may sit in the 126 MB L2: flush between steps
@@ -157,31 +159,38 @@ def run_ours(args, rank, world):
         if world > 1:
             torch.distributed.barrier()
 
+    def timed_steps():
+        """exactly args.steps steps, CUDA events on the library's stream; returns device ms"""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        barrier()
+        for k in range(args.steps):
+            if flush is not None:
+                flush.fill_(k & 1)
+            ev[k][0].record(stream)
+            ctx.step(w.dt)
+            ev[k][1].record(stream)
+        barrier()
+        ctx.sync()
+        if flush is not None:
+            return sum(a.elapsed_time(b) for a, b in ev)
+        return ev[0][0].elapsed_time(ev[-1][1])
+
     # ---- device-resident arm ----
     for _ in range(args.warmup):
-        ctx.step(w.dt)
+        ctx.step(w.dt)                       # the second step with the same dt captures the step graph
     ctx.sync()
-    ctx.timing_enable(True)
-    ctx.timing_read()
+    # region A: the headline time -- sph_step as the library runs it (graph replay), no brackets
     launches0 = ctx.launch_count()
     sampler = ClockSampler(local)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
     sampler.start()
-    for k in range(args.steps):
-        if flush is not None:
-            flush.fill_(k & 1)
-        ev[k][0].record()
-        ctx.step(w.dt)
-        ev[k][1].record()
-    barrier()
+    ms_dev = timed_steps()
     clocks = sampler.stop()
-    ctx.sync()
-    if flush is not None:
-        ms_dev = sum(a.elapsed_time(b) for a, b in ev)
-    else:
-        ms_dev = ev[0][0].elapsed_time(ev[-1][1])
     launches = ctx.launch_count() - launches0
+    # region B: the same steps with the library's CUDA-event brackets around every stage (plain
+    # launches: the brackets are not part of the graph) -- stage shares and the roofline kernel's time
+    ctx.timing_enable(True)
+    ctx.timing_read()
+    ms_bracketed = timed_steps()
     stages = ctx.timing_read()
     ctx.timing_enable(False)
     counters = ctx.get_counters()
@@ -217,7 +226,7 @@ def run_ours(args, rank, world):
 
     fp64_peak = P.sph_measure_fp64_peak()
     ctx.close()
-    return dict(w=w, ms_dev=ms_dev, launches=launches, stages=stages, counters=counters, clocks=clocks,
+    return dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters, clocks=clocks,
                 ms_e2e=ms_e2e, h2d=h2d, d2h=d2h, fp64_peak=fp64_peak, l2_flush=small, ws_bytes=ws_bytes,
                 t_gen=t_gen)
 
@@ -400,6 +409,9 @@ def main():
                 "l2": "L2 flushed (252 MB write) between timed steps" if r["l2_flush"]
                       else "working set larger than L2 (%.1f GB workspace)" % (r["ws_bytes"] / 1e9),
                 "particle_steps_per_s": n_total * args.steps / (ms_dev * 1e-3),
+                "timing": "value: K steps as the library runs them (sph_step replays its CUDA graph), CUDA events; "
+                          "stages/roofline: the same K steps again with per-stage CUDA-event brackets (plain launches)",
+                "ms_per_step_bracketed": r["ms_bracketed"] / args.steps,
                 "counters_last_eval": r["counters"]}),
             "clocks": r["clocks"],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(r["h2d"]),

@@ -4,6 +4,7 @@
 // gravity.cu; this file holds host logic and three small per-particle kernels (update, unsort).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -330,6 +331,10 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     cudaMemsetAsync(d.n_act, 0, n * sizeof(int), c->stream);
     cudaMemsetAsync(d.flaw_off, 0, (n + 1) * sizeof(i64), c->stream);
     cudaStreamSynchronize(c->stream);   // c->mats is pageable host memory: finish the copy now
+    sph_sort_init();
+    c->step_graph = nullptr;
+    c->last_dt = c->graph_dt = -1.0;
+    c->graphs_off = (getenv("SPH_NO_GRAPH") != nullptr);
     int rc = check_cuda(c, "sph_create");
     if (rc != SPH_OK) { delete e; return rc; }
     *out = c;
@@ -339,6 +344,7 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
 void sph_destroy(sph_ctx *ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
     delete ctx->timing;
     delete ext(ctx);
 }
@@ -460,9 +466,8 @@ int sph_evaluate(sph_ctx *ctx) {
     return sph_gravity(ctx);
 }
 
-int sph_step(sph_ctx *ctx, double dt) {
-    if (!ctx) return SPH_ERR_ARG;
-    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
+// the launches of one predictor-corrector step, enqueued on ctx->stream
+static int step_enqueue(sph_ctx *ctx, double dt) {
     Dev &d = ctx->d;
     const size_t n = (size_t)d.n;
     int rc;
@@ -484,6 +489,50 @@ int sph_step(sph_ctx *ctx, double dt) {
     }
     ctx->have_tree = ctx->have_lists = 0;   // the state moved on; the rates stay readable
     return check_cuda(ctx, "sph_step");
+}
+
+// A step is ~170 launches; for the small workloads (C1-C3) the GPU idles between them.  The launch
+// sequence of a step depends only on the configuration and on dt, so it is captured into a CUDA
+// graph the second time in a row a dt is asked for and replayed from then on (stage timing runs the
+// plain launches: event brackets are not part of the graph).
+int sph_step(sph_ctx *ctx, double dt) {
+    if (!ctx) return SPH_ERR_ARG;
+    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
+    if (ctx->timing || ctx->graphs_off) return step_enqueue(ctx, dt);
+    if (ctx->step_graph && ctx->graph_dt == dt) {
+        if (cudaGraphLaunch(ctx->step_graph, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
+        ctx->launches += ctx->graph_launches;
+        ctx->have_tree = ctx->have_lists = 0;
+        ctx->have_rates = 3;
+        return SPH_OK;
+    }
+    const bool repeat = (ctx->last_dt == dt);
+    ctx->last_dt = dt;
+    if (!repeat) return step_enqueue(ctx, dt);
+    if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->graphs_off = 1;
+        return step_enqueue(ctx, dt);
+    }
+    const i64 l0 = ctx->launches;
+    const int rc = step_enqueue(ctx, dt);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(ctx->stream, &graph);
+    cudaGraphExec_t exec = nullptr;
+    if (rc != SPH_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        ctx->launches = l0;
+        ctx->graphs_off = 1;                 // nothing has run: do the step with plain launches
+        return step_enqueue(ctx, dt);
+    }
+    cudaGraphDestroy(graph);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
+    ctx->step_graph = exec;
+    ctx->graph_dt = dt;
+    ctx->graph_launches = ctx->launches - l0;
+    if (cudaGraphLaunch(exec, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
+    return SPH_OK;
 }
 
 static int device_flags(sph_ctx *ctx) {

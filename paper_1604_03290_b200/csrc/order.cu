@@ -199,13 +199,13 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
     }
 }
 
+// one-time kernel attributes (called by sph_create, outside any stream capture)
+void sph_sort_init() {
+    cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+}
+
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur) {
     const int nblocks = sph_ceil_div(n_host, SORT_TILE);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
-        attr_set = true;
-    }
     int c = *cur;
     for (int shift = 0; shift < bits; shift += 8) {
         k_sort_hist<<<nblocks, 256, 0, ctx->stream>>>(key[c], n_host, n_dev, shift, ctx->d.hist, nblocks);

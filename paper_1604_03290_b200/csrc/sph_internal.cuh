@@ -141,6 +141,11 @@ struct sph_ctx {
     i64 launches;
     int sort_cur;
     SphTiming *timing;          // NULL unless sph_timing_enable(ctx, 1)
+    // sph_step as a CUDA graph: captured when the same dt is asked for twice in a row, replayed after
+    cudaGraphExec_t step_graph;
+    double graph_dt, last_dt;
+    i64 graph_launches;
+    int graphs_off;
     char err[512];
 };
 
@@ -162,6 +167,7 @@ static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 // (n_host) or, if n_dev != NULL, from device memory (kernels early-exit; grids sized for n_host).
 // Result ends in key[*cur], val[*cur].
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur);
+void sph_sort_init();
 
 // ---- scan.cu ---- exclusive prefix sums (in == out allowed); scratch[ceil(n/2048)] = grand total
 void sph_scan_u32(sph_ctx *ctx, const unsigned *in, unsigned *out, i64 n, unsigned *scratch);
