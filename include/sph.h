@@ -145,7 +145,12 @@ int sph_gravity(sph_ctx *ctx);
 /* One complete right-hand-side evaluation: build_tree, find_neighbours, rhs, gravity. */
 int sph_evaluate(sph_ctx *ctx);
 
-/* A12: predictor-corrector step (eqs. 52-53): two complete evaluations and two updates. */
+/* A12: predictor-corrector step (eqs. 52-53): two complete evaluations and two updates.
+ * The launch sequence of a step depends only on the configuration and dt: when the same dt is asked
+ * for twice in a row the library captures the sequence into a CUDA graph and replays it on later
+ * calls with that dt (same results bit for bit).  This needs a capturable stream (not the legacy
+ * default stream) and no stage timing; otherwise, or with SPH_NO_GRAPH set in the environment at
+ * sph_create, the kernels are launched one by one. */
 int sph_step(sph_ctx *ctx, double dt);
 
 /* Upper limits of the next time step from the rates of the LAST complete evaluation:
