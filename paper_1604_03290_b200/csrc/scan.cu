@@ -89,9 +89,36 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const T *in, T *out
     }
 }
 
+// small inputs (the digit tables of the radix sort for the small workloads): one block, one launch
+#define SCAN_SMALL 16384
+template <class T>
+__global__ void __launch_bounds__(1024) k_scan_small(const T *in, T *out, T *bsum, int n, int nb) {
+    __shared__ T s_warp[33];
+    __shared__ T s_run;
+    if (threadIdx.x == 0) s_run = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < n; b0 += 1024) {
+        const int i = b0 + threadIdx.x;
+        const T v = (i < n) ? in[i] : (T)0;
+        T tot;
+        const T ex = block_excl_scan(v, s_warp, &tot);
+        const T run = s_run;
+        if (i < n) out[i] = run + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) s_run = run + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) bsum[nb] = s_run;
+}
+
 template <class T>
 static void scan_impl(sph_ctx *ctx, const T *in, T *out, i64 n, T *bsum) {
     const int nb = sph_ceil_div(n, SCAN_TILE);
+    if (n <= SCAN_SMALL) {
+        k_scan_small<T><<<1, 1024, 0, ctx->stream>>>(in, out, bsum, (int)n, nb);
+        ctx->launches += 1;
+        return;
+    }
     k_scan_reduce<T><<<nb, SCAN_THREADS, 0, ctx->stream>>>(in, bsum, n);
     k_scan_sums<T><<<1, 1024, 0, ctx->stream>>>(bsum, nb);
     k_scan_apply<T><<<nb, SCAN_THREADS, 0, ctx->stream>>>(in, out, bsum, n);
