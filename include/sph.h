@@ -54,7 +54,8 @@ enum {
     SPH_F_VARIABLE_H = 16,   /* mean smoothing length per pair + eq. 73 update */
     SPH_F_DENSITY_SUM = 32,  /* rho by kernel sum, eq. 28, instead of continuity */
     SPH_F_ART_STRESS = 64,   /* artificial stress against the tensile instability (eqs. 35-38) */
-    SPH_F_XSPH = 128         /* particles move with the XSPH-smoothed velocity (eq. 40) */
+    SPH_F_XSPH = 128,        /* particles move with the XSPH-smoothed velocity (eq. 40) */
+    SPH_F_RK3 = 256          /* reserve the rate buffers of the embedded Runge-Kutta step (sph_step_rk3) */
 };
 
 enum { SPH_EOS_IDEAL_GAS = 0, SPH_EOS_MURNAGHAN = 1, SPH_EOS_TILLOTSON = 2 };
@@ -152,6 +153,17 @@ int sph_evaluate(sph_ctx *ctx);
  * default stream) and no stage timing; otherwise, or with SPH_NO_GRAPH set in the environment at
  * sph_create, the kernels are launched one by one. */
 int sph_step(sph_ctx *ctx, double dt);
+
+/* One step of the embedded Runge-Kutta scheme (eqs. 58-65): three complete
+ * evaluations k1 = f(q), k2 = f(q + dt/2 k1), k3 = f(q - dt k1 + 2 dt k2); third-order result
+ * q + dt (k1 + 4 k2 + k3)/6 (eq. 58), midpoint result q + dt k2 (eq. 62), error estimate
+ * eps_err = max |q_mm - q_rk3| / |q + dt k1| over all particles and integrated quantities with a
+ * non-zero denominator (eq. 63).  eps_err <= eps_des: the state becomes the third-order result and
+ * dt_new = dt |eps_des/eps_err|^0.3 (eq. 64); otherwise the state is left unchanged and
+ * dt_new = 0.9 dt |eps_des/eps_err|^(1/4) (eq. 65).  Stage states get the post-update rules of
+ * sph_step; n_act is committed (maximum over the three evaluations) only on acceptance.
+ * out (HOST double[3]) = eps_err, dt_new, accepted (1.0 / 0.0).  Needs SPH_F_RK3.  Synchronises. */
+int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out);
 
 /* Upper limits of the next time step from the rates of the LAST complete evaluation:
  *   out[0] = min_a 0.2 h_a / |dv_a/dt|       (eq. 54; the acceleration includes self-gravity)

@@ -441,3 +441,109 @@ def step(w, dt, mode="brute"):
     qn = advance(w, qp.v, f2, dt, f2["n_act"])
     qn.n_act = f2["n_act"].astype(np.int32)
     return qn, f1, f2
+
+
+# -----------------------------------------------------------------------------------------
+# Embedded Runge-Kutta integrator, PAPER.md:416-451 (eqs. 58-65)
+# -----------------------------------------------------------------------------------------
+def rk3_embedded(q, f, dt):
+    """eqs. 58-63 for a plain vector quantity q and a rate function f(q): returns (q_rk3, q_mm,
+    eps_err) with eps_err = max |q_mm - q_rk3| / |q + dt f(q)| over the entries whose denominator is
+    not zero (0 when there is none).  Used by the pins; step_rk3 applies the same formulas."""
+    k1 = f(q)                                            # eq. 59
+    k2 = f(q + 0.5 * dt * k1)                            # eq. 60
+    k3 = f(q - dt * k1 + 2.0 * dt * k2)                  # eq. 61
+    q_rk3 = q + dt * (k1 / 6.0 + 4.0 * k2 / 6.0 + k3 / 6.0)   # eq. 58
+    q_mm = q + dt * k2                                   # eq. 62
+    den = np.abs(q + dt * k1)                            # eq. 63
+    num = np.abs(q_mm - q_rk3)
+    ok = den > 0.0
+    return q_rk3, q_mm, (float(np.max(num[ok] / den[ok])) if ok.any() else 0.0)
+
+
+def rk3_new_dt(dt, eps_err, eps_des):
+    """eq. 64 (accepted: eps_err <= eps_des) and eq. 65 (rejected). Returns (accepted, dt_new)."""
+    if eps_err <= eps_des:
+        return True, (float("inf") if eps_err == 0.0 else dt * abs(eps_des / eps_err) ** 0.3)
+    return False, 0.9 * dt * abs(eps_des / eps_err) ** 0.25
+
+
+def _rk_fields(w):
+    """integrated quantities and the names of their rates (reading U29: every integrated quantity
+    enters the error estimate of eq. 63)"""
+    names = [("x", None), ("v", None), ("u", "du")]
+    if not (w.flags & F_DENSITY_SUM):
+        names.append(("rho", "drho"))
+    if w.flags & F_SOLID:
+        names.append(("S", "dS"))
+    if w.flags & F_DAMAGE:
+        names.append(("dmg", "ddmg"))
+    return names
+
+
+def _rk_rate(w, q, f, name, rate):
+    if name == "x":
+        return q.v + f["dxs"] if (w.flags & F_XSPH) else q.v          # eqs. 39 / 40
+    if name == "v":
+        return f["dv"] + f["ag"]
+    return f[rate]
+
+
+def step_rk3(w, dt, eps_des, mode="brute"):
+    """One step of the embedded Runge-Kutta scheme of PAPER.md:416-451 with the SPH right-hand side.
+    Stage states get the same post-update rules as the predictor of the RK2 scheme (damage clamp of
+    eq. 47 with the activated flaws of the evaluation that produced the newest rate, limiter of eq.
+    16); n_act is committed (maximum over the three evaluations) only when the step is accepted
+    (readings U29-U30).  Returns (state, eps_err, dt_new, accepted, [f1, f2, f3]); on rejection the
+    state is the unchanged input."""
+    D = w.dim
+    fields = _rk_fields(w)
+
+    def make_state(coeffs, ks, n_act_eval, f_last):
+        q = w.copy()
+        for name, _ in fields:
+            val = getattr(w, name).copy()
+            for c, k in zip(coeffs, ks):
+                val = val + (dt * c) * k[name]
+            setattr(q, name, val)
+        if w.flags & F_DENSITY_SUM:
+            q.rho = f_last["rho"].copy()
+        if w.flags & F_DAMAGE:
+            ntot = (w.flaw_off[1:] - w.flaw_off[:-1]).astype(np.float64)
+            dmax = np.cbrt(np.where(ntot > 0, n_act_eval / np.maximum(ntot, 1.0), 0.0))
+            q.dmg = np.minimum(np.maximum(q.dmg, 0.0), dmax)
+        q.h = f_last["h"].copy()
+        if D == 2:
+            q.x[2] = 0.0
+            q.v[2] = 0.0
+        _limit(q)
+        q.n_act = w.n_act.copy()
+        return q
+
+    def rates(q, f):
+        return {name: _rk_rate(w, q, f, name, rate) for name, rate in fields}
+
+    f1 = evaluate(w, mode)
+    k1 = rates(w, f1)
+    q2 = make_state([0.5], [k1], f1["n_act"], f1)                       # eq. 60
+    f2 = evaluate(q2, mode)
+    k2 = rates(q2, f2)
+    q3 = make_state([-1.0, 2.0], [k1, k2], f2["n_act"], f2)             # eq. 61
+    f3 = evaluate(q3, mode)
+    k3 = rates(q3, f3)
+    eps_err = 0.0
+    for name, _ in fields:                                               # eqs. 58, 62, 63 on the raw sums
+        q0 = getattr(w, name)
+        q_rk3 = q0 + dt * (k1[name] / 6.0 + 4.0 * k2[name] / 6.0 + k3[name] / 6.0)
+        q_mm = q0 + dt * k2[name]
+        den = np.abs(q0 + dt * k1[name])
+        ok = den > 0.0
+        if ok.any():
+            eps_err = max(eps_err, float(np.max(np.abs(q_mm - q_rk3)[ok] / den[ok])))
+    accepted, dt_new = rk3_new_dt(dt, eps_err, eps_des)
+    if not accepted:
+        return w.copy(), eps_err, dt_new, False, [f1, f2, f3]
+    n_act = np.maximum(np.maximum(f1["n_act"], f2["n_act"]), f3["n_act"]).astype(np.int32)
+    qn = make_state([1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0], [k1, k2, k3], n_act, f3)
+    qn.n_act = n_act
+    return qn, eps_err, dt_new, True, [f1, f2, f3]

@@ -18,13 +18,13 @@ SPH_OK = 0
 SPH_ERR_ARG, SPH_ERR_STATE, SPH_ERR_WORKSPACE = -1, -2, -3
 SPH_ERR_NEIGHBOUR_OVERFLOW, SPH_ERR_TREE_DEPTH, SPH_ERR_CUDA = -4, -5, -6
 SPH_F_SOLID, SPH_F_PLASTIC, SPH_F_DAMAGE, SPH_F_GRAVITY, SPH_F_VARIABLE_H, SPH_F_DENSITY_SUM = 1, 2, 4, 8, 16, 32
-SPH_F_ART_STRESS, SPH_F_XSPH = 64, 128
+SPH_F_ART_STRESS, SPH_F_XSPH, SPH_F_RK3 = 64, 128, 256
 
 EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sph_build_tree",
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
-           "sph_timing_name", "sph_get_counters", "sph_timestep", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+           "sph_timing_name", "sph_get_counters", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
 SPH_T_COUNT = 11
 
 _vp = C.c_void_p
@@ -104,6 +104,7 @@ def load_library():
     L.sph_timing_name.argtypes = [C.c_int]
     L.sph_get_counters.argtypes = [_vp, _vp]
     L.sph_timestep.argtypes = [_vp, _vp]
+    L.sph_step_rk3.argtypes = [_vp, C.c_double, C.c_double, _vp]
     L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
     L.sph_measure_copy_bw.argtypes = [_vp, _vp, _vp, C.c_size_t, C.POINTER(C.c_double)]
     _lib = L
@@ -307,6 +308,12 @@ class Context:
         self._check(L.sph_timing_read(self.handle, ms.ctypes.data, ln.ctypes.data))
         return {L.sph_timing_name(k).decode(): (float(ms[k]), int(ln[k])) for k in range(SPH_T_COUNT)}
 
+    def step_rk3(self, dt, eps_des):
+        """sph_step_rk3: returns (eps_err, dt_new, accepted)."""
+        out = np.zeros(3)
+        self._check(load_library().sph_step_rk3(self.handle, float(dt), float(eps_des), out.ctypes.data))
+        return float(out[0]), float(out[1]), bool(out[2])
+
     def timestep(self):
         """sph_timestep: dict of the limits of eqs. 54, 55, 57 and their minimum (eq. 56)."""
         out = np.zeros(4)
@@ -366,6 +373,10 @@ def sph_step(ctx, dt):
 
 def sph_download(ctx, fields=STATE_FIELDS + RATE_FIELDS, device=False, out=None):
     return ctx.download(fields, device, out)
+
+
+def sph_step_rk3(ctx, dt, eps_des):
+    return ctx.step_rk3(dt, eps_des)
 
 
 def sph_timestep(ctx):

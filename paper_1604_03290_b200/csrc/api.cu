@@ -67,6 +67,9 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.flaw_off = b.take<i64>(n + 1);
     z.flaw_eps = b.take<double>((size_t)std::max<int64_t>(c->n_flaws, 1));
     z.q0 = b.take<double>(15 * n);
+    for (int k = 0; k < 3; ++k) z.rk[k] = b.take<double>((c->flags & SPH_F_RK3) ? 15 * n : 1);
+    z.rk_nact = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
+    z.rk_nmax = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
     for (int a = 0; a < 3; ++a) { z.sx[a] = b.take<double>(n); z.sv[a] = b.take<double>(n); }
     z.sm = b.take<double>(n); z.srho = b.take<double>(n); z.su = b.take<double>(n);
     for (int k = 0; k < 6; ++k) z.sS[k] = b.take<double>(n);
@@ -239,6 +242,120 @@ __global__ void k_update(Dev d, const sph_material *mats, double c, int commit) 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// embedded Runge-Kutta step, PAPER.md:416-451 (eqs. 58-65)
+// ------------------------------------------------------------------------------------------------
+// rates of the last evaluation -> K (original order, the 15-array layout of the state block):
+// dx/dt = v (+ XSPH term, eq. 40), dv/dt = SPH + gravity, drho/dt, du/dt, dS/dt, d(dmg)/dt
+__global__ void k_rk_rates(Dev d, double *K, int first) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const size_t n = (size_t)d.n;
+    const int o = d.perm[i];
+    for (int a = 0; a < 3; ++a) {
+        double vel = 0.0, acc = 0.0;
+        if (a < d.D) {
+            vel = d.v[a][o];
+            if (d.flags & SPH_F_XSPH) vel = __dadd_rn(vel, d.dxs[a][i]);
+            acc = __dadd_rn(d.dv[a][i], d.ag[a][i]);
+        }
+        K[(size_t)a * n + o] = vel;
+        K[(size_t)(3 + a) * n + o] = acc;
+    }
+    K[6 * n + o] = (d.flags & SPH_F_DENSITY_SUM) ? 0.0 : d.drho[i];
+    K[7 * n + o] = d.du[i];
+    for (int k = 0; k < 6; ++k) K[(size_t)(8 + k) * n + o] = (d.flags & SPH_F_SOLID) ? d.dS[k][i] : 0.0;
+    K[14 * n + o] = (d.flags & SPH_F_DAMAGE) ? d.ddmg[i] : 0.0;
+    if (d.flags & SPH_F_DAMAGE) {
+        const int na = d.n_act_new[i];
+        d.rk_nact[o] = na;
+        d.rk_nmax[o] = first ? na : max(d.rk_nmax[o], na);
+    }
+}
+
+// state <- q0 + dt (c1 k1 + c2 k2 + c3 k3), term by term, every product and sum rounded separately;
+// then the post-update rules of the predictor-corrector (eq. 47 clamp, eq. 16 limiter).  nterms = 1
+// (eq. 60), 2 (eq. 61) or 3 (eq. 58, commit: n_act <- maximum over the three evaluations).
+__global__ void k_rk_stage(Dev d, const sph_material *mats, double dt, double c1, double c2, double c3, int nterms) {
+    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= d.n) return;
+    const size_t n = (size_t)d.n;
+    const double cc[3] = {__dmul_rn(dt, c1), __dmul_rn(dt, c2), __dmul_rn(dt, c3)};
+    auto comb = [&](int q) {
+        double val = d.q0[(size_t)q * n + o];
+        for (int t = 0; t < nterms; ++t) val = __dadd_rn(val, __dmul_rn(cc[t], d.rk[t][(size_t)q * n + o]));
+        return val;
+    };
+    const int D = d.D;
+    for (int a = 0; a < 3; ++a) {
+        d.x[a][o] = (a < D) ? comb(a) : 0.0;
+        d.v[a][o] = (a < D) ? comb(3 + a) : 0.0;
+    }
+    if (!(d.flags & SPH_F_DENSITY_SUM)) d.rho[o] = comb(6);
+    d.u[o] = comb(7);
+    const sph_material &mt = mats[d.mat[o]];
+    if (d.flags & SPH_F_SOLID) {
+        double S[6];
+        for (int k = 0; k < 6; ++k) S[k] = comb(8 + k);
+        if ((d.flags & SPH_F_PLASTIC) && mt.Y0 > 0.0) {
+            double SS;
+            if (D == 3) {
+                const double dg = __dadd_rn(__dadd_rn(__dmul_rn(S[0], S[0]), __dmul_rn(S[3], S[3])), __dmul_rn(S[5], S[5]));
+                const double of = __dadd_rn(__dadd_rn(__dmul_rn(S[1], S[1]), __dmul_rn(S[2], S[2])), __dmul_rn(S[4], S[4]));
+                SS = __dadd_rn(dg, __dmul_rn(2.0, of));
+            } else {
+                SS = __dadd_rn(__dadd_rn(__dmul_rn(S[0], S[0]), __dmul_rn(S[3], S[3])), __dmul_rn(2.0, __dmul_rn(S[1], S[1])));
+            }
+            const double J2 = __dmul_rn(0.5, SS), Y2 = __dmul_rn(mt.Y0, mt.Y0), J3 = __dmul_rn(3.0, J2);
+            if (J3 > Y2) {
+                const double fY = __ddiv_rn(Y2, J3);
+                for (int k = 0; k < 6; ++k) S[k] = __dmul_rn(S[k], fY);
+            }
+        }
+        for (int k = 0; k < 6; ++k) d.S[k][o] = S[k];
+    }
+    if (d.flags & SPH_F_DAMAGE) {
+        const i64 ntot = d.flaw_off[o + 1] - d.flaw_off[o];
+        const int nact = (nterms == 3) ? d.rk_nmax[o] : d.rk_nact[o];
+        const double dmax = (ntot > 0) ? cbrt((double)nact / (double)ntot) : 0.0;
+        d.dmg[o] = fmin(fmax(comb(14), 0.0), dmax);
+        if (nterms == 3) d.n_act[o] = nact;
+    }
+}
+
+// eq. 63: max over particles and integrated quantities of |q_mm - q_rk3| / |q + dt k1| (non-zero
+// denominators only); positive doubles order like their bit patterns -> atomicMax on u64
+__global__ void k_rk_err_init(Dev d) { d.status->rkerr = 0ull; }
+__global__ void __launch_bounds__(256) k_rk_err(Dev d, double dt) {
+    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t n = (size_t)d.n;
+    double e = 0.0;
+    if (o < d.n) {
+        for (int q = 0; q < 15; ++q) {
+            if ((q < 3 && q >= d.D) || (q >= 3 && q < 6 && q - 3 >= d.D)) continue;
+            if (q == 6 && (d.flags & SPH_F_DENSITY_SUM)) continue;
+            if (q >= 8 && q < 14 && !(d.flags & SPH_F_SOLID)) continue;
+            if (d.D == 2 && (q == 10 || q == 12 || q == 13)) continue;
+            if (q == 14 && !(d.flags & SPH_F_DAMAGE)) continue;
+            const double q0 = d.q0[(size_t)q * n + o], k1 = d.rk[0][(size_t)q * n + o];
+            const double k2 = d.rk[1][(size_t)q * n + o], k3 = d.rk[2][(size_t)q * n + o];
+            const double s = __dadd_rn(__dadd_rn(__ddiv_rn(k1, 6.0), __ddiv_rn(__dmul_rn(4.0, k2), 6.0)), __ddiv_rn(k3, 6.0));
+            const double q3 = __dadd_rn(q0, __dmul_rn(dt, s));                       // eq. 58
+            const double qm = __dadd_rn(q0, __dmul_rn(dt, k2));                      // eq. 62
+            const double den = fabs(__dadd_rn(q0, __dmul_rn(dt, k1)));
+            if (den > 0.0) e = fmax(e, __ddiv_rn(fabs(__dsub_rn(qm, q3)), den));     // eq. 63
+        }
+    }
+    for (int off = 16; off > 0; off >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, off));
+    __shared__ double s_e[8];
+    if ((threadIdx.x & 31) == 0) s_e[threadIdx.x >> 5] = e;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) e = fmax(e, s_e[w]);
+        atomicMax(&d.status->rkerr, (u64)__double_as_longlong(e));
+    }
+}
+
 // PAPER.md:396-414 (eqs. 54-57): time-step limits, one min-reduction over the particles (sorted order).
 // Positive doubles order like their bit patterns, so the block minima are combined with atomicMin on u64.
 __global__ void k_dtlim_init(Dev d) {
@@ -388,6 +505,48 @@ int sph_get_counters(sph_ctx *ctx, int64_t *out) {
     cudaStreamSynchronize(ctx->stream);
     out[0] = st.n_nodes; out[1] = (int64_t)st.n_pairs; out[2] = (int64_t)st.n_inter; out[3] = (int64_t)st.n_visit;
     return check_cuda(ctx, "sph_get_counters");
+}
+
+int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out) {
+    if (!ctx || !out) return SPH_ERR_ARG;
+    if (!(ctx->d.flags & SPH_F_RK3)) return fail(ctx, SPH_ERR_STATE, "sph_step_rk3 needs SPH_F_RK3 at sph_create");
+    if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step_rk3 before sph_upload");
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    const int gb = sph_ceil_div(d.n, 256);
+    int rc;
+    cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    const double c[3][3] = {{0.5, 0.0, 0.0}, {-1.0, 2.0, 0.0}, {1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0}};
+    for (int st = 0; st < 3; ++st) {
+        if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;                                   // eqs. 59-61
+        k_rk_rates<<<gb, 256, 0, ctx->stream>>>(d, d.rk[st], st == 0);
+        ctx->launches += 1;
+        if (st < 2) {
+            k_rk_stage<<<gb, 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, c[st][0], c[st][1], c[st][2], st + 1);
+            ctx->launches += 1;
+        }
+    }
+    k_rk_err_init<<<1, 1, 0, ctx->stream>>>(d);
+    k_rk_err<<<gb, 256, 0, ctx->stream>>>(d, dt);
+    ctx->launches += 2;
+    DevStatus stt;
+    cudaMemcpyAsync(&stt, d.status, sizeof(stt), cudaMemcpyDeviceToHost, ctx->stream);
+    cudaStreamSynchronize(ctx->stream);
+    double err;
+    memcpy(&err, &stt.rkerr, sizeof(double));
+    const bool ok = err <= eps_des;
+    if (ok) {
+        k_rk_stage<<<gb, 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, c[2][0], c[2][1], c[2][2], 3);   // eq. 58
+        ctx->launches += 1;
+        out[1] = (err == 0.0) ? INFINITY : dt * pow(fabs(eps_des / err), 0.3);               // eq. 64
+    } else {
+        cudaMemcpyAsync(d.x[0], d.q0, 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+        out[1] = 0.9 * dt * pow(fabs(eps_des / err), 0.25);                                 // eq. 65
+    }
+    out[0] = err;
+    out[2] = ok ? 1.0 : 0.0;
+    ctx->have_tree = ctx->have_lists = 0;
+    return check_cuda(ctx, "sph_step_rk3");
 }
 
 int sph_timestep(sph_ctx *ctx, double *out) {

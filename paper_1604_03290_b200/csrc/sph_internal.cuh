@@ -26,6 +26,7 @@ struct DevStatus {
     u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
     int n_items;        // records of the partner-search stream
     int pad;
+    u64 rkerr;          // bit pattern of the error estimate of eq. 63 (sph_step_rk3)
     u64 dtlim[3];       // bit patterns of the three time-step limits (positive doubles order like integers)
 };
 
@@ -83,6 +84,8 @@ struct Dev {
     double *flaw_eps;
     // ---- RK2 base copy (x v rho u S dmg: 15 arrays contiguous) ----
     double *q0;
+    double *rk[3];              // k1, k2, k3 of sph_step_rk3, original order, 15 arrays each (SPH_F_RK3)
+    int *rk_nact, *rk_nmax;     // activated flaws of the newest evaluation / maximum over the step
     // ---- sorted working copies ----
     double *sx[3], *sv[3], *sm, *srho, *su, *sS[6], *sdmg, *sh;
     int *smat;

@@ -37,6 +37,7 @@ F_VARIABLE_H = 16
 F_DENSITY_SUM = 32
 F_ART_STRESS = 64      # artificial stress, PAPER.md:284-302 (eqs. 35-38)
 F_XSPH = 128           # XSPH velocity smoothing, PAPER.md:311 (eq. 40)
+F_RK3 = 256            # library only: reserve the rate buffers of the embedded Runge-Kutta step
 
 EOS_IDEAL_GAS = 0
 EOS_MURNAGHAN = 1

@@ -393,3 +393,42 @@ def test_step_graph_replay_is_bit_identical(P, monkeypatch):
     assert la == lb
     for k in a:
         assert np.array_equal(a[k], b[k]), k
+
+
+@pytest.mark.parametrize("name", ["C1x-twin", "C4-twin", "C2-twin"])
+def test_step_rk3_parity(P, name):
+    """sph_step_rk3 (eqs. 58-65) against the oracle: error estimate, new step size, accepted state;
+    a rejected step leaves the state untouched."""
+    w = CASES[name]()
+    w.flags |= P.SPH_F_RK3
+    w0 = w.copy(); w0.h_iters = 0
+    qn, err_o, dt_o, ok_o, fs = orc.step_rk3(w0, w.dt, 1e30, mode="brute")
+    assert ok_o
+    ctx = make_ctx(P, w, h_iters=0)
+    err, dt_new, ok = ctx.step_rk3(w.dt, 1e30)
+    assert ok
+    assert err == pytest.approx(err_o, rel=1e-6)
+    assert dt_new == pytest.approx(dt_o, rel=1e-6)
+    g = ctx.download(P.STATE_FIELDS)
+    for k in ("x", "v", "rho", "u", "S", "dmg"):
+        go, oo = g[k], getattr(qn, k)
+        scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
+        assert np.all(np.abs(go - oo) <= 1e-9 * np.abs(oo) + 1e-12 * scale), k
+    assert np.mean(g["n_act"] == qn.n_act) > 0.999
+    ctx.close()
+    # rejection: eps_des far below the estimate
+    ctx = make_ctx(P, w, h_iters=0)
+    err2, dt2, ok2 = ctx.step_rk3(w.dt, 1e-30)
+    assert not ok2 and err2 == pytest.approx(err_o, rel=1e-6)
+    assert dt2 == pytest.approx(0.9 * w.dt * (1e-30 / err2) ** 0.25, rel=1e-12)
+    g = ctx.download(P.STATE_FIELDS)
+    for k in ("x", "v", "u", "S", "dmg"):
+        assert np.array_equal(g[k], getattr(w, k)), k
+    assert np.array_equal(g["n_act"], w.n_act)
+    ctx.close()
+    # without SPH_F_RK3 the call is refused
+    w.flags &= ~P.SPH_F_RK3
+    ctx = make_ctx(P, w, h_iters=0)
+    with pytest.raises(P.SphError):
+        ctx.step_rk3(w.dt, 1e-3)
+    ctx.close()

@@ -134,3 +134,39 @@ def test_timestep_limits_hand_values_and_scaling():
     # nobody limits: +inf
     e4 = dict(e); e4["du"] = np.zeros(n)
     assert orc.timestep(w, e4)["change"] == float("inf")
+
+
+# ------------------------------------------------------------------ embedded RK3
+def test_rk3_embedded_on_linear_ode_closed_forms():
+    """dq/dt = lam q: eq. 58 reproduces the Taylor polynomial to third order, eq. 62 to second, so
+    eq. 63 gives |z^3/6| / |1 + z| with z = lam dt; eqs. 64-65 by hand."""
+    lam = np.array([-0.7, 0.3, 1.9, -2.2])
+    q = np.array([1.3, -0.4, 2.5, 0.9])
+    dt = 0.21
+    z = lam * dt
+    q_rk3, q_mm, err = orc.rk3_embedded(q, lambda y: lam * y, dt)
+    assert np.allclose(q_rk3, q * (1 + z + z ** 2 / 2 + z ** 3 / 6), rtol=1e-14)
+    assert np.allclose(q_mm, q * (1 + z + z ** 2 / 2), rtol=1e-14)
+    assert err == pytest.approx(np.max(np.abs(z ** 3 / 6) / np.abs(1 + z)), rel=1e-12)
+    # third order: halving dt divides the one-step error by ~16 (local error ~ dt^4)
+    exact = lambda t: q * np.exp(lam * t)
+    e1 = np.abs(orc.rk3_embedded(q, lambda y: lam * y, dt)[0] - exact(dt)).max()
+    e2 = np.abs(orc.rk3_embedded(q, lambda y: lam * y, dt / 2)[0] - exact(dt / 2)).max()
+    assert 12.0 < e1 / e2 < 20.0
+    # zero denominators are skipped
+    assert orc.rk3_embedded(np.zeros(3), lambda y: 0.0 * y, dt)[2] == 0.0
+    # eqs. 64-65
+    assert orc.rk3_new_dt(0.1, 1e-4, 1e-3) == (True, pytest.approx(0.1 * 10 ** 0.3))
+    assert orc.rk3_new_dt(0.1, 1e-2, 1e-3) == (False, pytest.approx(0.9 * 0.1 * 0.1 ** 0.25))
+
+
+def test_step_rk3_accepts_and_rejects():
+    w = si.make("C1x", scale=0.05, twin=True)
+    q, err, dt_new, ok, fs = orc.step_rk3(w, w.dt, 1e30)
+    assert ok and err > 0.0 and dt_new > w.dt
+    q2, err2, dt2, ok2, _ = orc.step_rk3(w, w.dt, 1e-30)
+    assert not ok2 and err2 == err and dt2 < w.dt
+    assert np.array_equal(q2.x, w.x) and np.array_equal(q2.v, w.v) and np.array_equal(q2.S, w.S)
+    # the accepted state is close to the RK2 state (both at least second order)
+    q_rk2, _, _ = orc.step(w, w.dt)
+    assert np.abs(q.v - q_rk2.v).max() <= 1e-3 * np.abs(q_rk2.v).max()
