@@ -8,7 +8,9 @@
 //   * The search stream (built by sph_build_search_items below) holds, in depth-first pre-order,
 //     the octree cells with more than SPH_BUCKET particles and BUCKETS of <= SPH_BUCKET particles
 //     that are consecutive in Morton order (runs of small sibling cells / leaves).  Every record
-//     carries the tight bounding box and the largest h of the particles below it.
+//     carries the bounding box and the largest h of the particles below it, rounded OUTWARD to
+//     FP32: pruning runs on the FP32 pipe with directed rounding (a box that holds a partner is
+//     never cut), the FP64 pipe is kept for the exact membership tests.
 //   * Every lane keeps the index of the next record IT has to look at: a cell whose box is out
 //     of the lane's reach is skipped (next = skip index), otherwise entered (next = cur + 1).
 //     The warp visits min over lanes(next) (one redux.sync), so the records a warp touches are
