@@ -79,7 +79,9 @@ typedef struct {
     int32_t max_neighbours; /* capacity of one interaction list (PAPER.md:481 interactionsList); 0 = 128 */
     int32_t n_des;          /* desired partner count of eq. 73 */
     int32_t h_iters;        /* eq.-73 updates per sph_find_neighbours (only with SPH_F_VARIABLE_H) */
-    int32_t reserved;
+    int32_t gravity_every;  /* gravity/hydro decoupling: sph_step walks the tree for self-gravity only in
+                               every gravity_every-th step and reuses the stored accelerations in between; 0 or 1 =
+                               every step.  sph_gravity and sph_evaluate always walk. */
     int64_t n;              /* particles */
     int64_t n_flaws;        /* total flaw thresholds (length of flaw_eps); 0 without damage */
     double theta;           /* opening angle of eq. 50; must be < 1/sqrt(dim) */

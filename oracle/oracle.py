@@ -404,9 +404,11 @@ def _limit(w):
         w.S = S * fY[None, :]
 
 
-def step(w, dt, mode="brute"):
+def step(w, dt, mode="brute", ag_reuse=None):
     """Predictor-corrector, PAPER.md:388-394 (eqs. 52-53): two full RHS evaluations.
-    Returns the new workload state (a copy) and the two evaluations."""
+    Returns the new workload state (a copy) and the two evaluations.
+    ag_reuse (3, n): gravity/hydro decoupling (reading U31) -- both evaluations take this
+    stored gravitational acceleration instead of walking the tree."""
     D = w.dim
 
     def advance(base, vel, f, c, n_act_eval):
@@ -435,9 +437,13 @@ def step(w, dt, mode="brute"):
         return q
 
     f1 = evaluate(w, mode)
+    if ag_reuse is not None:
+        f1["ag"] = np.array(ag_reuse, dtype=np.float64)
     qp = advance(w, w.v, f1, 0.5 * dt, f1["n_act"])
     qp.n_act = w.n_act.copy()                            # committed only after the corrector (U19)
     f2 = evaluate(qp, mode)
+    if ag_reuse is not None:
+        f2["ag"] = np.array(ag_reuse, dtype=np.float64)
     qn = advance(w, qp.v, f2, dt, f2["n_act"])
     qn.n_act = f2["n_act"].astype(np.int32)
     return qn, f1, f2

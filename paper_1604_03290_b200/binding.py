@@ -37,7 +37,7 @@ class Material(C.Structure):
 
 class Config(C.Structure):
     _fields_ = [("dim", C.c_int32), ("flags", C.c_int32), ("n_materials", C.c_int32), ("morton_bits", C.c_int32),
-                ("max_neighbours", C.c_int32), ("n_des", C.c_int32), ("h_iters", C.c_int32), ("reserved", C.c_int32),
+                ("max_neighbours", C.c_int32), ("n_des", C.c_int32), ("h_iters", C.c_int32), ("gravity_every", C.c_int32),
                 ("n", C.c_int64), ("n_flaws", C.c_int64), ("theta", C.c_double), ("G", C.c_double),
                 ("eps_soft", C.c_double), ("av_alpha", C.c_double), ("av_beta", C.c_double), ("av_eps", C.c_double),
                 ("as_eps", C.c_double), ("as_n", C.c_double), ("as_mpd", C.c_double), ("xsph", C.c_double)]
@@ -113,9 +113,9 @@ def load_library():
 
 def make_config(dim, n, flags, n_materials=1, morton_bits=21, max_neighbours=128, n_des=50, h_iters=0,
                 n_flaws=0, theta=0.5, G=0.0, eps_soft=0.0, av_alpha=1.0, av_beta=0.0, av_eps=0.01,
-                as_eps=0.2, as_n=4.0, as_mpd=1.0, xsph=0.5):
+                as_eps=0.2, as_n=4.0, as_mpd=1.0, xsph=0.5, gravity_every=0):
     return Config(dim=dim, flags=flags, n_materials=n_materials, morton_bits=morton_bits,
-                  max_neighbours=max_neighbours, n_des=n_des, h_iters=h_iters, reserved=0, n=n, n_flaws=n_flaws,
+                  max_neighbours=max_neighbours, n_des=n_des, h_iters=h_iters, gravity_every=gravity_every, n=n, n_flaws=n_flaws,
                   theta=theta, G=G, eps_soft=eps_soft, av_alpha=av_alpha, av_beta=av_beta, av_eps=av_eps,
                   as_eps=as_eps, as_n=as_n, as_mpd=as_mpd, xsph=xsph)
 
@@ -128,12 +128,12 @@ def make_materials(materials):
     return arr
 
 
-def config_of(w, h_iters=None, max_neighbours=None, morton_bits=21):
+def config_of(w, h_iters=None, max_neighbours=None, morton_bits=21, gravity_every=0):
     """sph_config + materials of a workload object from sph_inputs (plain field copy)."""
     cfg = make_config(w.dim, w.n, w.flags, len(w.materials), morton_bits,
                       w.max_neighbours if max_neighbours is None else max_neighbours, w.n_des,
                       w.h_iters if h_iters is None else h_iters, int(w.flaw_eps.size), w.theta, w.G, w.eps_soft,
-                      w.av_alpha, w.av_beta, w.av_eps, w.as_eps, w.as_n, w.as_mpd, w.xsph)
+                      w.av_alpha, w.av_beta, w.av_eps, w.as_eps, w.as_n, w.as_mpd, w.xsph, gravity_every)
     return cfg, make_materials(w.materials)
 
 

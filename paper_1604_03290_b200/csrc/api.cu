@@ -37,7 +37,7 @@ bool cfg_ok(const sph_config *c) {
     if (c->n_materials < 1 || c->n_materials > SPH_MAX_MAT) return false;
     if (c->morton_bits < 0 || c->morton_bits > 21) return false;
     if (c->max_neighbours < 0 || c->max_neighbours > 4096) return false;
-    if (c->n_flaws < 0) return false;
+    if (c->n_flaws < 0 || c->gravity_every < 0) return false;
     if ((c->flags & SPH_F_GRAVITY) && !(c->theta >= 0.0 && c->theta * c->theta * c->dim < 1.0)) return false;
     if ((c->flags & SPH_F_VARIABLE_H) && c->h_iters > 0 && c->n_des < 1) return false;
     if ((c->flags & SPH_F_ART_STRESS) && !(c->as_mpd > 0.0 && c->as_n > 0.0 && c->as_eps >= 0.0)) return false;
@@ -68,6 +68,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.flaw_eps = b.take<double>((size_t)std::max<int64_t>(c->n_flaws, 1));
     z.q0 = b.take<double>(15 * n);
     for (int k = 0; k < 3; ++k) z.rk[k] = b.take<double>((c->flags & SPH_F_RK3) ? 15 * n : 1);
+    for (int a = 0; a < 3; ++a) z.ag_keep[a] = b.take<double>((c->gravity_every > 1) ? n : 1);
     z.rk_nact = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
     z.rk_nmax = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
     for (int a = 0; a < 3; ++a) { z.sx[a] = b.take<double>(n); z.sv[a] = b.take<double>(n); }
@@ -356,6 +357,20 @@ __global__ void __launch_bounds__(256) k_rk_err(Dev d, double dt) {
     }
 }
 
+// gravity/hydro decoupling (reading U31): keep / take the walked accelerations, original order
+__global__ void k_ag_keep(Dev d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const int o = d.perm[i];
+    for (int a = 0; a < 3; ++a) d.ag_keep[a][o] = d.ag[a][i];
+}
+__global__ void k_ag_take(Dev d) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const int o = d.perm[i];
+    for (int a = 0; a < 3; ++a) d.ag[a][i] = d.ag_keep[a][o];
+}
+
 // PAPER.md:396-414 (eqs. 54-57): time-step limits, one min-reduction over the particles (sorted order).
 // Positive doubles order like their bit patterns, so the block minima are combined with atomicMin on u64.
 __global__ void k_dtlim_init(Dev d) {
@@ -581,6 +596,7 @@ int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
     cp(d.flaw_eps, s->flaw_eps, (size_t)ctx->cfg.n_flaws * 8);
     if (!src_is_device) cudaStreamSynchronize(ctx->stream);   // caller may free or reuse its buffers
     ctx->have_state = 1; ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
+    ctx->step_no = 0;
     return check_cuda(ctx, "sph_upload");
 }
 
@@ -622,6 +638,13 @@ int sph_evaluate(sph_ctx *ctx) {
     if ((rc = sph_build_tree(ctx)) != SPH_OK) return rc;
     if ((rc = sph_find_neighbours(ctx)) != SPH_OK) return rc;
     if ((rc = sph_rhs(ctx)) != SPH_OK) return rc;
+    if (ctx->grav_reuse) {                   // decoupled step: the stored field, brought into the new order
+        StageTimer tm(ctx, SPH_T_GRAVITY);
+        k_ag_take<<<sph_ceil_div(ctx->d.n, 256), 256, 0, ctx->stream>>>(ctx->d);
+        ctx->launches += 1;
+        ctx->have_rates |= 2;
+        return check_cuda(ctx, "sph_evaluate");
+    }
     return sph_gravity(ctx);
 }
 
@@ -630,17 +653,26 @@ static int step_enqueue(sph_ctx *ctx, double dt) {
     Dev &d = ctx->d;
     const size_t n = (size_t)d.n;
     int rc;
+    const int every = ctx->cfg.gravity_every;
+    const bool decoupled = every > 1 && (d.flags & SPH_F_GRAVITY);
+    ctx->grav_reuse = decoupled && (ctx->step_no % every) != 0;
+    ctx->step_no += 1;
     {
         StageTimer tm(ctx, SPH_T_UPDATE);
         cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
     }
-    if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
+    if ((rc = sph_evaluate(ctx)) != SPH_OK) { ctx->grav_reuse = 0; return rc; }
     {
         StageTimer tm(ctx, SPH_T_UPDATE);
         k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), 0.5 * dt, 0);   // eq. 52
         ctx->launches += 1;
     }
-    if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
+    if ((rc = sph_evaluate(ctx)) != SPH_OK) { ctx->grav_reuse = 0; return rc; }
+    if (decoupled && !ctx->grav_reuse) {     // the field the next gravity_every - 1 steps reuse
+        k_ag_keep<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
+        ctx->launches += 1;
+    }
+    ctx->grav_reuse = 0;
     {
         StageTimer tm(ctx, SPH_T_UPDATE);
         k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, 1);         // eq. 53
@@ -657,7 +689,7 @@ static int step_enqueue(sph_ctx *ctx, double dt) {
 int sph_step(sph_ctx *ctx, double dt) {
     if (!ctx) return SPH_ERR_ARG;
     if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
-    if (ctx->timing || ctx->graphs_off) return step_enqueue(ctx, dt);
+    if (ctx->timing || ctx->graphs_off || ctx->cfg.gravity_every > 1) return step_enqueue(ctx, dt);
     if (ctx->step_graph && ctx->graph_dt == dt) {
         if (cudaGraphLaunch(ctx->step_graph, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
         ctx->launches += ctx->graph_launches;

@@ -85,6 +85,7 @@ struct Dev {
     // ---- RK2 base copy (x v rho u S dmg: 15 arrays contiguous) ----
     double *q0;
     double *rk[3];              // k1, k2, k3 of sph_step_rk3, original order, 15 arrays each (SPH_F_RK3)
+    double *ag_keep[3];         // last walked gravitational acceleration, original order (gravity_every > 1)
     int *rk_nact, *rk_nmax;     // activated flaws of the newest evaluation / maximum over the step
     // ---- sorted working copies ----
     double *sx[3], *sv[3], *sm, *srho, *su, *sS[6], *sdmg, *sh;
@@ -149,6 +150,8 @@ struct sph_ctx {
     double graph_dt, last_dt;
     i64 graph_launches;
     int graphs_off;
+    i64 step_no;                // sph_step calls since the last upload (gravity_every)
+    int grav_reuse;             // set by sph_step: sph_evaluate takes the stored accelerations
     char err[512];
 };
 

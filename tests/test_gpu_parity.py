@@ -432,3 +432,30 @@ def test_step_rk3_parity(P, name):
     with pytest.raises(P.SphError):
         ctx.step_rk3(w.dt, 1e-3)
     ctx.close()
+
+
+def test_gravity_hydro_decoupling(P):
+    """gravity_every = 2 (reading U31): steps 0 and 2 walk the tree, step 1 reuses the
+    accelerations of step 0's corrector evaluation; the oracle is given the same stored field."""
+    w = CASES["C5-twin"]()
+    cfg, mats = P.config_of(w, h_iters=0, gravity_every=2)
+    ctx = P.sph_create(cfg, mats)
+    ctx.upload_workload(w)
+    q = w.copy(); q.h_iters = 0
+    keep = None
+    for s in range(3):
+        ctx.step(w.dt)
+        if s % 2 == 0:
+            q, f1, f2 = orc.step(q, w.dt, mode="brute")
+            keep = f2["ag"].copy()
+        else:
+            q, f1, f2 = orc.step(q, w.dt, mode="brute", ag_reuse=keep)
+        q.h_iters = 0
+        g = ctx.download()
+        for k in ("x", "v", "rho", "u", "S", "dmg"):
+            go, oo = g[k], getattr(q, k)
+            scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
+            assert np.all(np.abs(go - oo) <= 1e-8 * np.abs(oo) + 1e-11 * scale), (s, k)
+        # the acceleration left in the context is the walked or the stored one
+        assert_close(f"ag(step {s})", g["ag"], f2["ag"], rel=1e-8, floor=1e-11 * np.abs(f2["ag"]).max())
+    ctx.close()
