@@ -459,3 +459,43 @@ def test_gravity_hydro_decoupling(P):
         # the acceleration left in the context is the walked or the stored one
         assert_close(f"ag(step {s})", g["ag"], f2["ag"], rel=1e-8, floor=1e-11 * np.abs(f2["ag"]).max())
     ctx.close()
+
+
+def test_coarse_morton_keys_many_particles_per_leaf(P):
+    """morton_bits = 3: most leaves of the octree hold several particles (equal keys at the deepest
+    level) -- the multi-particle-leaf paths of the tree build, the partner search and the gravity walk."""
+    w = sph_inputs.random_blob(3000, dim=3, seed=21)
+    L = 3
+    ctx = make_ctx(P, w, morton_bits=L)
+    ctx.evaluate()
+    ctx.sync()
+    tree = orc.Tree(w, L=L)
+    okey, operm = tree.order()
+    keys, perm, root = ctx.get_order()
+    assert np.array_equal(keys, okey) and np.array_equal(perm, operm)
+    assert np.unique(keys).size < 0.7 * w.n                      # equal keys do occur
+    on, gn = tree.nodes(), canonical(ctx.get_tree())
+    for k in ("level", "prefix", "lo", "hi", "mass"):
+        assert np.array_equal(gn[k], on[k]), k
+    off_o, idx_o = orc.neighbours(w, mode="brute")               # partner sets do not depend on the keys
+    check_neighbours(ctx, off_o, idx_o)
+    ag, A, _ = orc.gravity_tree(w, tree=tree)
+    g = ctx.download(("ag",))["ag"]
+    assert_close("ag", g, ag, A)
+    ctx.close()
+
+
+def test_partial_upload_keeps_the_other_fields(P):
+    w = CASES["blob3d"]()
+    ctx = make_ctx(P, w)
+    x2 = w.x * 1.01
+    ctx.upload(x=x2)                                             # NULL members are left unchanged
+    ctx.evaluate()
+    g = ctx.download()
+    w2 = w.copy(); w2.x = x2
+    ref = make_ctx(P, w2)
+    ref.evaluate()
+    r = ref.download()
+    for k in g:
+        assert np.array_equal(g[k], r[k]), k
+    ctx.close(); ref.close()
