@@ -16,7 +16,10 @@
 // passages carry the U-numbers of SURVEY.md section 8(c) / DESIGN.md "Readings".
 //
 // Parity pins: every function here is pinned by tests/test_oracle_*.py (closed forms,
-// invariants, brute force) EXCEPT the two readings the paper cannot pin:
+// invariants, brute force, golden values of tests/golden/; round 2 added the sign of S in
+// eqs. 30/31, the (1-d) S factor of eq. 20, a hand value of Tillotson eq. 15, the density sum
+// with the mean h, and the post-update rules of the step in tests/test_oracle_pins_r2.py)
+// EXCEPT the readings the paper cannot pin:
 //   * crack growth speed c_g and the length R_s in eqs. 24/46 (U16): "parity unpinned"
 //     by the paper (pinned only by dimensional analysis and the hand-computed formula);
 //   * the per-component tension criterion of the artificial stress, eq. 37 (U25): "parity

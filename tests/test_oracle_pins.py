@@ -435,7 +435,7 @@ def test_gravity_theta_zero_is_direct_sum_and_theta_half_error():
     # north_star asks for a median relative error <= 1e-3 at theta = 0.5.  The paper's method
     # (monopoles only, s/r < theta on the geometric cell edge) does not reach
     # that at 0.5: measured 3.3e-3 / 2.6e-3 / 2.3e-3 at N = 3277 / 16384 / 65536 (DESIGN.md,
-    # reading R-G1).  It does at theta = 0.3, and the error grows like theta^2 or faster
+    # reading U32).  It does at theta = 0.3, and the error grows like theta^2 or faster
     # ("The error scales with theta^2").
     assert rel3 <= 1e-3
     assert rel5 <= 5e-3
