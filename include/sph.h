@@ -42,7 +42,8 @@ enum {
     SPH_ERR_STATE = -2,              /* call order: e.g. sph_rhs before sph_find_neighbours */
     SPH_ERR_WORKSPACE = -3,          /* workspace too small or misaligned (256 B) */
     SPH_ERR_NEIGHBOUR_OVERFLOW = -4, /* a particle has more than max_neighbours partners */
-    SPH_ERR_TREE_DEPTH = -5,         /* traversal stack exhausted (too many particles share one key) */
+    SPH_ERR_TREE_DEPTH = -5,         /* gravity walk: traversal stack exhausted (a guard: the pop policy bounds the stack for
+                                        every theta and particle distribution, see csrc/gravity.cu) */
     SPH_ERR_CUDA = -6                /* CUDA runtime error or no device; see sph_last_error */
 };
 
@@ -55,7 +56,9 @@ enum {
     SPH_F_DENSITY_SUM = 32,  /* rho by kernel sum, eq. 28, instead of continuity */
     SPH_F_ART_STRESS = 64,   /* artificial stress against the tensile instability (eqs. 35-38) */
     SPH_F_XSPH = 128,        /* particles move with the XSPH-smoothed velocity (eq. 40) */
-    SPH_F_RK3 = 256          /* reserve the rate buffers of the embedded Runge-Kutta step (sph_step_rk3) */
+    SPH_F_RK3 = 256,         /* reserve the rate buffers of the embedded Runge-Kutta step (sph_step_rk3) */
+    SPH_F_EXPORT_GRADV = 512 /* keep the velocity gradient of eq. 42 and the correction tensor of eqs. 43-44 of the last
+                                evaluation (18 n doubles more workspace) so that sph_download can return them */
 };
 
 enum { SPH_EOS_IDEAL_GAS = 0, SPH_EOS_MURNAGHAN = 1, SPH_EOS_TILLOTSON = 2 };
@@ -109,12 +112,17 @@ typedef struct {
  * gravitational acceleration), p and cs (equation of state), strain (eq. 48), n_act_new (activated
  * flaws found by the last evaluation, latched with the committed count), nb_count (partners),
  * dxs (eq. 40: the XSPH term x_sph sum_b 2 m_b/(rho_a+rho_b) (v_b - v_a) W_ab, so that dx/dt = v + dxs;
- * zero without SPH_F_XSPH). */
+ * zero without SPH_F_XSPH); gradv[3*alpha+beta] = d v^alpha / d x^beta of eq. 42 and C[3*gamma+beta] = the
+ * correction tensor of eqs. 43-44 (identity where reading U17 applies), both only with
+ * SPH_F_SOLID | SPH_F_EXPORT_GRADV, zero otherwise.
+ * With HOST buffers the rates are un-sorted by one kernel into workspace that sph_step and sph_rhs also use,
+ * copied out, and the call synchronises once. */
 typedef struct {
     double *x[3], *v[3], *rho, *u, *S[6], *dmg, *h;
     double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *p, *cs, *strain;
     int32_t *n_act, *n_act_new, *nb_count;
     double *dxs[3];
+    double *gradv[9], *C[9];
 } sph_state_out;
 
 /* Bytes of device workspace sph_create needs for this configuration (0 on invalid config). */
@@ -127,7 +135,8 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
 void sph_destroy(sph_ctx *ctx);
 
 /* Copy particle state into the context (original order). src_is_device: 1 = DEVICE pointers,
- * 0 = HOST pointers (pinned memory makes the copy asynchronous). Invalidates tree and lists. */
+ * 0 = HOST pointers (pinned memory makes the copy asynchronous). Invalidates tree and lists and clears
+ * the device-side failures latched by evaluations of the previous state. */
 int sph_upload(sph_ctx *ctx, const sph_state_in *src, int src_is_device);
 
 /* A1-A4: bounding cube (eq. 67) -> Morton keys -> radix sort + SoA reorder -> octree topology ->
@@ -164,6 +173,9 @@ int sph_step(sph_ctx *ctx, double dt);
  * dt_new = dt |eps_des/eps_err|^0.3 (eq. 64); otherwise the state is left unchanged and
  * dt_new = 0.9 dt |eps_des/eps_err|^(1/4) (eq. 65).  Stage states get the post-update rules of
  * sph_step; n_act is committed (maximum over the three evaluations) only on acceptance.
+ * A rejected step gives back the whole state, including the smoothing lengths that eq. 73 rewrote during the
+ * three evaluations.  A state or rate that is not finite gives eps_err = +inf: rejected, dt_new = 0.
+ * A device-side failure of one of the evaluations (list overflow) is returned and nothing is accepted.
  * out (HOST double[3]) = eps_err, dt_new, accepted (1.0 / 0.0).  Needs SPH_F_RK3.  Synchronises. */
 int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out);
 
@@ -173,7 +185,9 @@ int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out);
  *   out[2] = min_a,q 0.7 |q_a| / |dq_a/dt|   (eq. 57) over q = rho (not with SPH_F_DENSITY_SUM), u, the
  *            components of S (SPH_F_SOLID) and dmg (SPH_F_DAMAGE); entries with q = 0 or dq/dt = 0 are skipped
  *   out[3] = the smallest of the three       (eq. 56 with eq. 57)
- * A limit that no particle sets is +infinity.  out: HOST double[4].  Synchronises. */
+ * A limit that no particle sets is +infinity; a NaN state or rate gives the limit 0.  Without SPH_F_GRAVITY
+ * (or before sph_gravity) eq. 54 takes the SPH acceleration alone.  out: HOST double[4].  Synchronises and
+ * reports device-side failures of the evaluation. */
 int sph_timestep(sph_ctx *ctx, double *out);
 
 /* Copy state and/or the rates of the last evaluation out, original order.
@@ -226,7 +240,8 @@ int sph_timing_read(sph_ctx *ctx, double *ms, int64_t *launches);
 const char *sph_timing_name(int stage);
 /* Work counters of the LAST evaluation (HOST out[4]; synchronises): internal nodes; sum over
  * particles of the partner count; sum over particles of gravity interactions (accepted pseudo-
- * particles + directly summed particles, eq. 51); sum over particles of opening tests (eq. 50). */
+ * particles + directly summed particles, eq. 51); sum over particles of opening tests (eq. 50: accepted
+ * and opened cells).  Also reports device-side failures of the evaluation. */
 int sph_get_counters(sph_ctx *ctx, int64_t *out);
 /* Dependency-free FP64 FMA throughput of the device [TFLOP/s] (the ALU roofline denominator;
  * MEASURED_PEAKS.json has no FP64 figure). stream: cudaStream_t. Synchronises. */

@@ -18,7 +18,7 @@ SPH_OK = 0
 SPH_ERR_ARG, SPH_ERR_STATE, SPH_ERR_WORKSPACE = -1, -2, -3
 SPH_ERR_NEIGHBOUR_OVERFLOW, SPH_ERR_TREE_DEPTH, SPH_ERR_CUDA = -4, -5, -6
 SPH_F_SOLID, SPH_F_PLASTIC, SPH_F_DAMAGE, SPH_F_GRAVITY, SPH_F_VARIABLE_H, SPH_F_DENSITY_SUM = 1, 2, 4, 8, 16, 32
-SPH_F_ART_STRESS, SPH_F_XSPH, SPH_F_RK3 = 64, 128, 256
+SPH_F_ART_STRESS, SPH_F_XSPH, SPH_F_RK3, SPH_F_EXPORT_GRADV = 64, 128, 256, 512
 
 EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sph_build_tree",
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
@@ -52,11 +52,11 @@ class StateOut(C.Structure):
     _fields_ = [("x", _vp * 3), ("v", _vp * 3), ("rho", _vp), ("u", _vp), ("S", _vp * 6), ("dmg", _vp), ("h", _vp),
                 ("drho", _vp), ("dv", _vp * 3), ("du", _vp), ("dS", _vp * 6), ("ddmg", _vp), ("ag", _vp * 3),
                 ("p", _vp), ("cs", _vp), ("strain", _vp), ("n_act", _vp), ("n_act_new", _vp), ("nb_count", _vp),
-                ("dxs", _vp * 3)]
+                ("dxs", _vp * 3), ("gradv", _vp * 9), ("C", _vp * 9)]
 
 
 _OUT_SHAPES = dict(x=3, v=3, rho=0, u=0, S=6, dmg=0, h=0, drho=0, dv=3, du=0, dS=6, ddmg=0, ag=3, p=0, cs=0,
-                   strain=0, n_act=0, n_act_new=0, nb_count=0, dxs=3)
+                   strain=0, n_act=0, n_act_new=0, nb_count=0, dxs=3, gradv=9, C=9)
 _OUT_INT = ("n_act", "n_act_new", "nb_count")
 STATE_FIELDS = ("x", "v", "rho", "u", "S", "dmg", "h", "n_act")
 RATE_FIELDS = ("drho", "dv", "du", "dS", "ddmg", "ag", "p", "cs", "strain", "n_act_new", "nb_count", "dxs")

@@ -71,6 +71,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     for (int a = 0; a < 3; ++a) z.ag_keep[a] = b.take<double>((c->gravity_every > 1) ? n : 1);
     z.rk_nact = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
     z.rk_nmax = b.take<int>((c->flags & SPH_F_RK3) ? n : 1);
+    z.h0 = b.take<double>((c->flags & SPH_F_RK3) ? n : 1);
     for (int a = 0; a < 3; ++a) { z.sx[a] = b.take<double>(n); z.sv[a] = b.take<double>(n); }
     z.sm = b.take<double>(n); z.srho = b.take<double>(n); z.su = b.take<double>(n);
     for (int k = 0; k < 6; ++k) z.sS[k] = b.take<double>(n);
@@ -107,6 +108,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(n);
     z.n_act_new = b.take<int>(n);
     for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? n : 1);
+    for (int k = 0; k < 9; ++k) { z.gradv[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? n : 1); z.Cten[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? n : 1); }
     z.stage = b.take<double>(n);
     z.stage_i = b.take<int>(n);
     Mats *md = b.take<Mats>(1);
@@ -125,6 +127,17 @@ int check_cuda(sph_ctx *ctx, const char *where) {
     if (e == cudaSuccess) return SPH_OK;
     snprintf(ctx->err, sizeof(ctx->err), "%s: %s", where, cudaGetErrorString(e));
     return SPH_ERR_CUDA;
+}
+
+// Device-side failures latched by the kernels of the evaluations since the last sph_upload (which
+// clears them): every call that has the status block on the host reports them.
+int status_flags(sph_ctx *ctx, const DevStatus &st, const char *where) {
+    if (st.err_nb_overflow) {
+        snprintf(ctx->err, sizeof(ctx->err), "interaction list overflow: %d partners > max_neighbours %d", st.nb_max, ctx->d.cap);
+        return SPH_ERR_NEIGHBOUR_OVERFLOW;
+    }
+    if (st.err_stack) return fail(ctx, SPH_ERR_TREE_DEPTH, "gravity walk: traversal stack exhausted (internal bound violated)");
+    return check_cuda(ctx, where);
 }
 
 }  // namespace
@@ -173,13 +186,17 @@ const sph_material *sph_dev_mats(sph_ctx *ctx) { return ext(ctx)->mats_dev->m; }
 // ------------------------------------------------------------------------------------------------
 // small per-particle kernels
 // ------------------------------------------------------------------------------------------------
-__global__ void k_unsort_d(const double *__restrict__ src, const int *__restrict__ perm, double *__restrict__ dst, int n) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[perm[i]] = src[i];
-}
-__global__ void k_unsort_i(const int *__restrict__ src, const int *__restrict__ perm, int *__restrict__ dst, int n) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[perm[i]] = src[i];
+// Un-sort up to UJ_MAX arrays in one launch (blockIdx.y = array): dst[perm[i]] = src[i].
+#define UJ_MAX 48
+struct UJob { const void *src; void *dst; int is_int; int pad; };
+struct UJobs { UJob j[UJ_MAX]; };
+__global__ void k_unsort_many(UJobs jobs, const int *__restrict__ perm, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const UJob jb = jobs.j[blockIdx.y];
+    const int o = perm[i];
+    if (jb.is_int) ((int *)jb.dst)[o] = ((const int *)jb.src)[i];
+    else ((double *)jb.dst)[o] = ((const double *)jb.src)[i];
 }
 __global__ void k_fill_d(double *dst, double v, size_t n) {
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -330,6 +347,7 @@ __global__ void k_rk_err_init(Dev d) { d.status->rkerr = 0ull; }
 __global__ void __launch_bounds__(256) k_rk_err(Dev d, double dt) {
     const int o = blockIdx.x * blockDim.x + threadIdx.x;
     const size_t n = (size_t)d.n;
+    const double inf = __longlong_as_double(0x7ff0000000000000ll);
     double e = 0.0;
     if (o < d.n) {
         for (int q = 0; q < 15; ++q) {
@@ -344,7 +362,9 @@ __global__ void __launch_bounds__(256) k_rk_err(Dev d, double dt) {
             const double q3 = __dadd_rn(q0, __dmul_rn(dt, s));                       // eq. 58
             const double qm = __dadd_rn(q0, __dmul_rn(dt, k2));                      // eq. 62
             const double den = fabs(__dadd_rn(q0, __dmul_rn(dt, k1)));
-            if (den > 0.0) e = fmax(e, __ddiv_rn(fabs(__dsub_rn(qm, q3)), den));     // eq. 63
+            const double num = fabs(__dsub_rn(qm, q3));
+            if (!(den == den) || !(num == num) || isinf(den) || isinf(num)) e = inf;  // a state or rate that blew up: reject
+            else if (den > 0.0) e = fmax(e, __ddiv_rn(num, den));                      // eq. 63
         }
     }
     for (int off = 16; off > 0; off >>= 1) e = fmax(e, __shfl_xor_sync(0xffffffffu, e, off));
@@ -376,19 +396,23 @@ __global__ void k_ag_take(Dev d) {
 __global__ void k_dtlim_init(Dev d) {
     if (threadIdx.x < 3) d.status->dtlim[threadIdx.x] = 0x7ff0000000000000ull;
 }
-__global__ void __launch_bounds__(256) k_dtlim(Dev d) {
+__global__ void __launch_bounds__(256) k_dtlim(Dev d, int with_ag) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const double inf = __longlong_as_double(0x7ff0000000000000ll);
     double t[3] = {inf, inf, inf};
     if (i < d.n) {
         const double h = d.sh[i];
         double a2 = 0.0;
-        for (int a = 0; a < d.D; ++a) { const double acc = d.dv[a][i] + d.ag[a][i]; a2 += acc * acc; }
-        if (a2 > 0.0) t[0] = 0.2 * h / sqrt(a2);                       // eq. 54
+        for (int a = 0; a < d.D; ++a) { const double acc = with_ag ? d.dv[a][i] + d.ag[a][i] : d.dv[a][i]; a2 += acc * acc; }
+        // a NaN state or rate gives the limit 0 (fmin would drop it and the blow-up would go unseen)
+        if (!(a2 == a2)) t[0] = 0.0;
+        else if (a2 > 0.0) t[0] = 0.2 * h / sqrt(a2);                  // eq. 54
         const double cs = d.cs[i];
-        if (cs > 0.0) t[1] = 0.7 * h / cs;                              // eq. 55
+        if (!(cs == cs)) t[1] = 0.0;
+        else if (cs > 0.0) t[1] = 0.7 * h / cs;                         // eq. 55
         auto lim = [&](double q, double dq) {                          // eq. 57
-            if (q != 0.0 && dq != 0.0) t[2] = fmin(t[2], 0.7 * fabs(q) / fabs(dq));
+            if (!(q == q) || !(dq == dq)) t[2] = 0.0;
+            else if (q != 0.0 && dq != 0.0) t[2] = fmin(t[2], 0.7 * fabs(q) / fabs(dq));
         };
         if (!(d.flags & SPH_F_DENSITY_SUM)) lim(d.srho[i], d.drho[i]);
         lim(d.su[i], d.du[i]);
@@ -462,6 +486,7 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     cudaMemsetAsync(d.mat, 0, n * sizeof(int), c->stream);
     cudaMemsetAsync(d.n_act, 0, n * sizeof(int), c->stream);
     cudaMemsetAsync(d.flaw_off, 0, (n + 1) * sizeof(i64), c->stream);
+    for (int a = 0; a < 3; ++a) cudaMemsetAsync(d.ag[a], 0, n * sizeof(double), c->stream);   // read as 0 until a walk fills it
     cudaStreamSynchronize(c->stream);   // c->mats is pageable host memory: finish the copy now
     sph_sort_init();
     c->step_graph = nullptr;
@@ -519,7 +544,7 @@ int sph_get_counters(sph_ctx *ctx, int64_t *out) {
     cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
     cudaStreamSynchronize(ctx->stream);
     out[0] = st.n_nodes; out[1] = (int64_t)st.n_pairs; out[2] = (int64_t)st.n_inter; out[3] = (int64_t)st.n_visit;
-    return check_cuda(ctx, "sph_get_counters");
+    return status_flags(ctx, st, "sph_get_counters");
 }
 
 int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out) {
@@ -531,6 +556,9 @@ int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out) {
     const int gb = sph_ceil_div(d.n, 256);
     int rc;
     cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    // eq. 73 rewrites the master h in every evaluation: a rejected step must give it back too
+    const bool keep_h = (d.flags & SPH_F_VARIABLE_H) && ctx->cfg.h_iters > 0;
+    if (keep_h) cudaMemcpyAsync(d.h0, d.h, n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
     const double c[3][3] = {{0.5, 0.0, 0.0}, {-1.0, 2.0, 0.0}, {1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0}};
     for (int st = 0; st < 3; ++st) {
         if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;                                   // eqs. 59-61
@@ -547,16 +575,23 @@ int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out) {
     DevStatus stt;
     cudaMemcpyAsync(&stt, d.status, sizeof(stt), cudaMemcpyDeviceToHost, ctx->stream);
     cudaStreamSynchronize(ctx->stream);
+    if ((rc = status_flags(ctx, stt, "sph_step_rk3")) != SPH_OK) {          // truncated lists / walk: nothing is accepted
+        cudaMemcpyAsync(d.x[0], d.q0, 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+        if (keep_h) cudaMemcpyAsync(d.h, d.h0, n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+        ctx->have_tree = ctx->have_lists = 0;
+        return rc;
+    }
     double err;
     memcpy(&err, &stt.rkerr, sizeof(double));
-    const bool ok = err <= eps_des;
+    const bool ok = err <= eps_des;                                          // false for +inf (a NaN state or rate)
     if (ok) {
         k_rk_stage<<<gb, 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, c[2][0], c[2][1], c[2][2], 3);   // eq. 58
         ctx->launches += 1;
         out[1] = (err == 0.0) ? INFINITY : dt * pow(fabs(eps_des / err), 0.3);               // eq. 64
     } else {
         cudaMemcpyAsync(d.x[0], d.q0, 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
-        out[1] = 0.9 * dt * pow(fabs(eps_des / err), 0.25);                                 // eq. 65
+        if (keep_h) cudaMemcpyAsync(d.h, d.h0, n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+        out[1] = 0.9 * dt * pow(fabs(eps_des / err), 0.25);                                 // eq. 65 (0 when err = +inf)
     }
     out[0] = err;
     out[2] = ok ? 1.0 : 0.0;
@@ -570,14 +605,14 @@ int sph_timestep(sph_ctx *ctx, double *out) {
         return fail(ctx, SPH_ERR_STATE, "sph_timestep before a complete evaluation");
     Dev &d = ctx->d;
     k_dtlim_init<<<1, 32, 0, ctx->stream>>>(d);
-    k_dtlim<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
+    k_dtlim<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, (ctx->have_rates & 2) ? 1 : 0);
     ctx->launches += 2;
     DevStatus st;
     cudaMemcpyAsync(&st, d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
     cudaStreamSynchronize(ctx->stream);
     for (int k = 0; k < 3; ++k) memcpy(&out[k], &st.dtlim[k], sizeof(double));
     out[3] = std::min(out[0], std::min(out[1], out[2]));
-    return check_cuda(ctx, "sph_timestep");
+    return status_flags(ctx, st, "sph_timestep");
 }
 
 int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
@@ -594,6 +629,8 @@ int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
     cp(d.mat, s->mat, n * 4); cp(d.n_act, s->n_act, n * 4);
     cp(d.flaw_off, s->flaw_off, (n + 1) * 8);
     cp(d.flaw_eps, s->flaw_eps, (size_t)ctx->cfg.n_flaws * 8);
+    // a new state: the failures latched by evaluations of the old one no longer apply
+    cudaMemsetAsync(&d.status->err_nb_overflow, 0, 3 * sizeof(int), ctx->stream);   // err_nb_overflow, err_stack, nb_max
     if (!src_is_device) cudaStreamSynchronize(ctx->stream);   // caller may free or reuse its buffers
     ctx->have_state = 1; ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
     ctx->step_no = 0;
@@ -729,14 +766,11 @@ int sph_step(sph_ctx *ctx, double dt) {
 static int device_flags(sph_ctx *ctx) {
     DevStatus st;
     if (cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream) != cudaSuccess ||
-        cudaStreamSynchronize(ctx->stream) != cudaSuccess)
-        return check_cuda(ctx, "status") == SPH_OK ? SPH_ERR_CUDA : SPH_ERR_CUDA;
-    if (st.err_nb_overflow) {
-        snprintf(ctx->err, sizeof(ctx->err), "interaction list overflow: %d partners > max_neighbours %d", st.nb_max, ctx->d.cap);
-        return SPH_ERR_NEIGHBOUR_OVERFLOW;
+        cudaStreamSynchronize(ctx->stream) != cudaSuccess) {
+        check_cuda(ctx, "status");
+        return SPH_ERR_CUDA;
     }
-    if (st.err_stack) return fail(ctx, SPH_ERR_TREE_DEPTH, "traversal stack exhausted");
-    return check_cuda(ctx, "sync");
+    return status_flags(ctx, st, "sync");
 }
 
 int sph_sync(sph_ctx *ctx) {
@@ -758,53 +792,68 @@ int sph_download(sph_ctx *ctx, const sph_state_out *o, int dst_is_device) {
     plain(o->rho, d.rho, nb); plain(o->u, d.u, nb); plain(o->dmg, d.dmg, nb); plain(o->h, d.h, nb);
     for (int k = 0; k < 6; ++k) plain(o->S[k], d.S[k], nb);
     plain(o->n_act, d.n_act, (size_t)n * 4);
-    const bool want_rates = o->drho || o->dv[0] || o->dv[1] || o->dv[2] || o->du || o->ddmg || o->ag[0] || o->ag[1] ||
-                            o->ag[2] || o->p || o->cs || o->strain || o->n_act_new || o->nb_count || o->dS[0] ||
-                            o->dS[1] || o->dS[2] || o->dS[3] || o->dS[4] || o->dS[5] || o->dxs[0] || o->dxs[1] || o->dxs[2];
+    bool want_rates = o->drho || o->du || o->ddmg || o->p || o->cs || o->strain || o->n_act_new || o->nb_count;
+    for (int a = 0; a < 3; ++a) want_rates = want_rates || o->dv[a] || o->ag[a] || o->dxs[a];
+    for (int k = 0; k < 6; ++k) want_rates = want_rates || o->dS[k];
+    for (int k = 0; k < 9; ++k) want_rates = want_rates || o->gradv[k] || o->C[k];
     if (want_rates && !ctx->have_rates) return fail(ctx, SPH_ERR_STATE, "sph_download of rates before an evaluation");
-    const int gb = sph_ceil_div(n, 256);
-    auto unsort_d = [&](double *dst, const double *src, bool present) {
-        if (!dst) return;
-        if (!present) {   // quantity not computed under the current flags: zeros
-            if (dst_is_device) { k_fill_d<<<gb, 256, 0, ctx->stream>>>(dst, 0.0, (size_t)n); ctx->launches += 1; }
-            else memset(dst, 0, nb);
-            return;
-        }
-        if (dst_is_device) {
-            k_unsort_d<<<gb, 256, 0, ctx->stream>>>(src, d.perm, dst, n);
-        } else {
-            k_unsort_d<<<gb, 256, 0, ctx->stream>>>(src, d.perm, d.stage, n);
-            cudaMemcpyAsync(dst, d.stage, nb, cudaMemcpyDeviceToHost, ctx->stream);
-            cudaStreamSynchronize(ctx->stream);   // stage is reused by the next member
-        }
-        ctx->launches += 1;
-    };
-    auto unsort_i = [&](int *dst, const int *src, bool present) {
-        if (!dst) return;
-        if (!present) {
-            if (dst_is_device) cudaMemsetAsync(dst, 0, (size_t)n * 4, ctx->stream);
-            else memset(dst, 0, (size_t)n * 4);
-            return;
-        }
-        if (dst_is_device) {
-            k_unsort_i<<<gb, 256, 0, ctx->stream>>>(src, d.perm, dst, n);
-        } else {
-            k_unsort_i<<<gb, 256, 0, ctx->stream>>>(src, d.perm, d.stage_i, n);
-            cudaMemcpyAsync(dst, d.stage_i, (size_t)n * 4, cudaMemcpyDeviceToHost, ctx->stream);
-            cudaStreamSynchronize(ctx->stream);
-        }
-        ctx->launches += 1;
-    };
     const bool sph = (ctx->have_rates & 1) != 0, grav = (ctx->have_rates & 2) != 0;
     const bool solid = sph && (d.flags & SPH_F_SOLID), dam = sph && (d.flags & SPH_F_DAMAGE);
-    unsort_d(o->drho, d.drho, sph); unsort_d(o->du, d.du, sph);
-    for (int a = 0; a < 3; ++a) { unsort_d(o->dv[a], d.dv[a], sph); unsort_d(o->ag[a], d.ag[a], grav); }
-    for (int a = 0; a < 3; ++a) unsort_d(o->dxs[a], d.dxs[a], sph && (d.flags & SPH_F_XSPH));
-    for (int k = 0; k < 6; ++k) unsort_d(o->dS[k], d.dS[k], solid);
-    unsort_d(o->ddmg, d.ddmg, dam); unsort_d(o->strain, d.strain, dam);
-    unsort_d(o->p, d.p, sph); unsort_d(o->cs, d.cs, sph);
-    unsort_i(o->n_act_new, d.n_act_new, dam);
-    unsort_i(o->nb_count, d.nb_cnt, ctx->have_lists || sph);
+    const bool gexp = solid && (d.flags & SPH_F_EXPORT_GRADV);
+    // The rates live in Morton order: ONE kernel un-sorts every requested array (straight into the
+    // caller's DEVICE buffers, or into staging slots that are then copied to the HOST buffers), and a
+    // host download synchronises once.  Staging = the RK2 base copy q0 (15 n doubles, live only inside
+    // sph_step) followed by the pair records prec (16 n doubles, live only inside sph_rhs).
+    UJobs jobs;
+    struct Copy { void *dst; const void *src; size_t bytes; };
+    Copy copies[UJ_MAX];
+    int nj = 0;
+    size_t slot = 0;
+    auto stage_slot = [&](size_t k) -> double * {
+        return (k < 15) ? d.q0 + k * (size_t)n : d.prec + (k - 15) * (size_t)n;
+    };
+    auto job = [&](void *dst, const void *src, bool present, bool is_int) {
+        if (!dst) return;
+        const size_t bytes = (size_t)n * (is_int ? 4 : 8);
+        if (!present) {          // quantity not computed under the current flags: zeros
+            if (dst_is_device) cudaMemsetAsync(dst, 0, bytes, ctx->stream);
+            else memset(dst, 0, bytes);
+            return;
+        }
+        void *target = dst;
+        if (!dst_is_device) {
+            target = stage_slot(slot++);
+            copies[nj] = Copy{dst, target, bytes};
+        }
+        jobs.j[nj] = UJob{src, target, is_int ? 1 : 0, 0};
+        ++nj;
+    };
+    job(o->drho, d.drho, sph, false); job(o->du, d.du, sph, false);
+    for (int a = 0; a < 3; ++a) { job(o->dv[a], d.dv[a], sph, false); job(o->ag[a], d.ag[a], grav, false); }
+    for (int a = 0; a < 3; ++a) job(o->dxs[a], d.dxs[a], sph && (d.flags & SPH_F_XSPH), false);
+    for (int k = 0; k < 6; ++k) job(o->dS[k], d.dS[k], solid, false);
+    job(o->ddmg, d.ddmg, dam, false); job(o->strain, d.strain, dam, false);
+    job(o->p, d.p, sph, false); job(o->cs, d.cs, sph, false);
+    job(o->n_act_new, d.n_act_new, dam, true);
+    job(o->nb_count, d.nb_cnt, ctx->have_lists || sph, true);
+    if (nj > 0) {
+        dim3 grid(sph_ceil_div(n, 256), nj);
+        k_unsort_many<<<grid, 256, 0, ctx->stream>>>(jobs, d.perm, n);
+        ctx->launches += 1;
+        if (!dst_is_device)
+            for (int k = 0; k < nj; ++k) cudaMemcpyAsync(copies[k].dst, copies[k].src, copies[k].bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    }
+    // second batch: velocity gradient and correction tensor (18 arrays; the staging slots are free again
+    // only after the copies above, which are stream-ordered)
+    nj = 0; slot = 0;
+    for (int k = 0; k < 9; ++k) { job(o->gradv[k], d.gradv[k], gexp, false); job(o->C[k], d.Cten[k], gexp, false); }
+    if (nj > 0) {
+        dim3 grid(sph_ceil_div(n, 256), nj);
+        k_unsort_many<<<grid, 256, 0, ctx->stream>>>(jobs, d.perm, n);
+        ctx->launches += 1;
+        if (!dst_is_device)
+            for (int k = 0; k < nj; ++k) cudaMemcpyAsync(copies[k].dst, copies[k].src, copies[k].bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    }
     if (!dst_is_device) return device_flags(ctx);
     return check_cuda(ctx, "sph_download");
 }

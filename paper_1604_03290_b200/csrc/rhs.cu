@@ -16,8 +16,6 @@
 //               (eqs. 8, 10), dS/dt (eqs. 7, 9), Grady-Kipp damage (eqs. 46-49, 24).
 #include "sph_internal.cuh"
 
-struct DevMats { const sph_material *m; };
-
 __device__ __forceinline__ void eos_eval(const sph_material &mt, double rho, double u, double &p, double &cs) {
     if (mt.eos == SPH_EOS_IDEAL_GAS) {
         p = (mt.gamma - 1.0) * rho * u;
@@ -405,6 +403,9 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
         }
         d.dS[0][i] = dS[0][0]; d.dS[1][i] = dS[0][1]; d.dS[2][i] = dS[0][2];
         d.dS[3][i] = dS[1][1]; d.dS[4][i] = dS[1][2]; d.dS[5][i] = dS[2][2];
+        if (d.flags & SPH_F_EXPORT_GRADV) {                   // A8 made visible: eqs. 42-44 compared directly by the parity tests
+            for (int a = 0; a < 3; ++a) for (int c = 0; c < 3; ++c) { d.gradv[3 * a + c][i] = gv[a][c]; d.Cten[3 * a + c][i] = C[a][c]; }
+        }
     }
 
     // ---- Grady-Kipp damage, eqs. 46-49, 24 (readings U16, U18-U20) ----

@@ -87,6 +87,7 @@ struct Dev {
     double *rk[3];              // k1, k2, k3 of sph_step_rk3, original order, 15 arrays each (SPH_F_RK3)
     double *ag_keep[3];         // last walked gravitational acceleration, original order (gravity_every > 1)
     int *rk_nact, *rk_nmax;     // activated flaws of the newest evaluation / maximum over the step
+    double *h0;                 // smoothing lengths at the start of sph_step_rk3 (given back when the step is rejected)
     // ---- sorted working copies ----
     double *sx[3], *sv[3], *sm, *srho, *su, *sS[6], *sdmg, *sh;
     int *smat;
@@ -126,6 +127,7 @@ struct Dev {
     // ---- rates, sorted order ----
     double *drho, *dv[3], *du, *dS[6], *ddmg, *ag[3], *strain;
     double *dxs[3];             // XSPH term of eq. 40 (only with SPH_F_XSPH)
+    double *gradv[9], *Cten[9]; // velocity gradient (eq. 42) and correction tensor (eq. 43), row-major (only with SPH_F_EXPORT_GRADV)
     int *n_act_new;
     // ---- staging ----
     double *stage;              // n doubles, for unsorting downloads
@@ -164,8 +166,6 @@ struct StageTimer {
     ~StageTimer() { if (c->timing) sph_timing_end(c, stage); }
 };
 
-#define SPH_LAUNCH(ctx) ((ctx)->launches++)
-
 static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 
 // ---- sort.cu ----
@@ -186,7 +186,6 @@ void sph_stage_tree(sph_ctx *ctx);      // A3 + A4
 void sph_stage_neigh(sph_ctx *ctx);     // A5
 void sph_stage_rhs(sph_ctx *ctx);       // A6-A10
 void sph_stage_gravity(sph_ctx *ctx);   // A11
-void sph_stage_update(sph_ctx *ctx, double c, int commit);   // A12 (one of the two updates)
 void sph_stage_writeback_h(sph_ctx *ctx);
 void sph_launch_moments(sph_ctx *ctx, int hmax_only);   // tree.cu: pseudo-particles bottom-up, one launch
 

@@ -26,11 +26,20 @@ def P():
     return P
 
 
-def make_ctx(P, w, **kw):
+def make_ctx(P, w, export=False, **kw):
     cfg, mats = P.config_of(w, **kw)
+    if export:                                   # keep grad v and C of the last evaluation (A8 compared directly)
+        cfg.flags |= P.SPH_F_EXPORT_GRADV
     ctx = P.sph_create(cfg, mats)
     ctx.upload_workload(w)
     return ctx
+
+
+ALL_FIELDS = None
+
+
+def all_fields(P):
+    return P.STATE_FIELDS + P.RATE_FIELDS + ("gradv", "C")
 
 
 def assert_close(name, g, o, A=None, rel=REL, abs_a=ABS_A, floor=0.0):
@@ -90,6 +99,19 @@ def check_rates(w, g, o, targets=None):
     assert_close("dv", g["dv"][:, t], o["dv"], o["A_dv"])
     if w.flags & orc.F_SOLID:
         assert_close("dS", g["dS"][:, t], o["dS"], o["A_dS"])
+        if "gradv" in g:
+            # A8 directly (eqs. 42-44): the correction tensor C = N^-1 and the corrected velocity
+            # gradient.  C carries the conditioning of the moment matrix N: delta C ~ cond(N) * delta N.
+            Cg, Co = g["C"][:, t].T.reshape(-1, 3, 3), o["C"].T.reshape(-1, 3, 3)
+            No = np.linalg.inv(Co)
+            nrm = lambda M: np.sqrt((M * M).sum(axis=(1, 2)))
+            tol = 1e-12 * nrm(Co) * nrm(No) * nrm(Co)
+            errC = np.abs(Cg - Co).max(axis=(1, 2))
+            ident_o = np.all(Co == np.eye(3), axis=(1, 2))
+            ident_g = np.all(Cg == np.eye(3), axis=(1, 2))
+            assert np.array_equal(ident_o, ident_g), "reading U17 (C = identity) applied to different particles"
+            assert np.all(errC <= tol), f"C: {np.count_nonzero(errC > tol)} particles outside tolerance, worst {np.max(errC / tol):.3g} x"
+            assert_close("gradv", g["gradv"][:, t], o["gradv"], o["A_gradv"], abs_a=1e-12)
     if w.flags & orc.F_GRAVITY:
         assert_close("ag", g["ag"][:, t], o["ag"], o["A_ag"])
     if w.flags & orc.F_DENSITY_SUM:
@@ -116,6 +138,14 @@ def check_rates(w, g, o, targets=None):
             assert np.any(np.abs(eps - s) <= 1e-12 * abs(s)), f"n_act differs at particle {a} away from a tie"
         same = na_g == na_o
         assert_close("ddmg", g["ddmg"][t][same], o["ddmg"][same], rel=1e-10)
+
+
+def n_act_tie_zone(w, na_g, na_o, strain_o, rel=1e-9):
+    """Activated-flaw counts after a step: equal except where a threshold lies within `rel` of the oracle's strain
+    (the trajectory bound of the step tests; per evaluation the bar is 1e-12, see check_rates)."""
+    for a in np.flatnonzero(na_g != na_o):
+        eps = w.flaw_eps[w.flaw_off[a]:w.flaw_off[a + 1]]
+        assert np.any(np.abs(eps - strain_o[a]) <= rel * abs(strain_o[a])), f"n_act differs at particle {a} away from a tie"
 
 
 def _with_art(w):
@@ -145,15 +175,24 @@ def test_full_evaluation_parity_small(P, name):
     """Sizes the O(N^2) oracle finishes in seconds; several 32-particle groups, tiles and a ragged tail."""
     w = CASES[name]()
     assert w.n % 32 != 0 or name.startswith("blob")
-    ctx = make_ctx(P, w, h_iters=0)
+    ctx = make_ctx(P, w, export=True, h_iters=0)
     ctx.evaluate()
     ctx.sync()
     check_order_and_tree(P, ctx, w)
     o = orc.evaluate(w, mode="brute", h_iters=0)
     check_neighbours(ctx, o["nb_off"], o["nb_idx"])
-    g = ctx.download()
+    g = ctx.download(all_fields(P))
     assert np.array_equal(g["nb_count"], np.diff(o["nb_off"]))
     check_rates(w, g, o)
+    if not (w.flags & orc.F_SOLID):
+        assert not g["gradv"].any() and not g["C"].any()
+    # the same kernels without the export flag give the same rates bit for bit
+    plain = make_ctx(P, w, h_iters=0)
+    plain.evaluate()
+    gp = plain.download()
+    for k in gp:
+        assert np.array_equal(gp[k], g[k]), k
+    plain.close()
     # purity: an evaluation never changes x, v, u, S, dmg, n_act (rho only under DENSITY_SUM)
     for k in ("x", "v", "u", "S", "dmg"):
         assert np.array_equal(g[k], getattr(w, k)), k
@@ -234,7 +273,7 @@ def test_step_parity(P, name):
         go, oo = g[k], getattr(qn, k)
         scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
         assert np.all(np.abs(go - oo) <= 1e-9 * np.abs(oo) + 1e-12 * scale), k
-    assert np.mean(g["n_act"] == qn.n_act) > 0.999
+    n_act_tie_zone(w, g["n_act"], qn.n_act, f2["strain"])
     # the rates left in the context are those of the second evaluation (at the predicted state)
     assert_close("dv(step)", g["dv"], f2["dv"], f2["A_dv"], rel=1e-8, abs_a=1e-11)
     # multi-step protocol: download the GPU state, hand it to the oracle, compare that evaluation
@@ -414,7 +453,7 @@ def test_step_rk3_parity(P, name):
         go, oo = g[k], getattr(qn, k)
         scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
         assert np.all(np.abs(go - oo) <= 1e-9 * np.abs(oo) + 1e-12 * scale), k
-    assert np.mean(g["n_act"] == qn.n_act) > 0.999
+    n_act_tie_zone(w, g["n_act"], qn.n_act, np.maximum(np.maximum(fs[0]["strain"], fs[1]["strain"]), fs[2]["strain"]), rel=1e-8)
     ctx.close()
     # rejection: eps_des far below the estimate
     ctx = make_ctx(P, w, h_iters=0)
@@ -499,3 +538,97 @@ def test_partial_upload_keeps_the_other_fields(P):
     for k in g:
         assert np.array_equal(g[k], r[k]), k
     ctx.close(); ref.close()
+
+
+@pytest.mark.parametrize("theta", [0.1, 0.2])
+def test_gravity_stack_bound_small_theta(P, theta):
+    """with 70 k uniform particles and a small opening angle the walk opens far more cells than at
+    theta = 0.5; the pop policy of the gravity kernel (multi-pop only while a depth-first tail still fits) must keep
+    the shared-memory stack within bounds and the accelerations complete."""
+    n = 70000
+    rng = np.random.default_rng(77)
+    x = rng.uniform(0.0, 1.0, (3, n))
+    w = sph_inputs.Workload(name="uniform", dim=3, flags=sph_inputs.F_GRAVITY, materials=[sph_inputs.GAS], x=x,
+                            v=np.zeros((3, n)), m=rng.uniform(0.5, 1.5, n) / n, rho=np.ones(n), u=np.ones(n),
+                            S=np.zeros((6, n)), dmg=np.zeros(n), h=np.full(n, 0.01), mat=np.zeros(n, np.int32),
+                            n_act=np.zeros(n, np.int32), flaw_off=np.zeros(n + 1, np.int64), flaw_eps=np.zeros(0),
+                            theta=theta, G=1.0, eps_soft=1e-3)
+    ctx = make_ctx(P, w)
+    ctx.build_tree()
+    ctx.gravity()
+    ctx.sync()                                            # raises on err_stack
+    g = ctx.download(("ag",))["ag"]
+    t = np.sort(rng.choice(n, 400, replace=False))
+    ag, A, ni = orc.gravity_tree(w, targets=t)
+    assert_close("ag", g[:, t], ag, A)
+    assert ni.mean() > 4000                               # many more interactions than at theta = 0.5
+    ctx.close()
+
+
+def test_rk3_rejection_gives_back_h(P):
+    """with SPH_F_VARIABLE_H and h_iters > 0 every evaluation rewrites the master h (eq. 73); a rejected
+    sph_step_rk3 must leave the state, h included, bit-identical."""
+    w = sph_inputs.c2_gas_sphere(n=2000)
+    w.h = w.h * np.random.default_rng(5).uniform(0.85, 1.2, w.n)
+    w.flags |= P.SPH_F_RK3
+    ctx = make_ctx(P, w, h_iters=1)
+    err, dt_new, ok = ctx.step_rk3(w.dt, 1e-30)
+    assert not ok and err > 0
+    g = ctx.download(P.STATE_FIELDS)
+    for k in ("x", "v", "u", "h"):
+        assert np.array_equal(g[k], getattr(w, k)), k
+    # and the retry with the smaller step starts from the same h: identical to a fresh context
+    e1 = ctx.step_rk3(dt_new, 1e30)
+    ref = make_ctx(P, w, h_iters=1)
+    e2 = ref.step_rk3(dt_new, 1e30)
+    assert e1 == e2
+    a, b = ctx.download(P.STATE_FIELDS), ref.download(P.STATE_FIELDS)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    ctx.close(); ref.close()
+
+
+def test_latched_failures_are_reported_and_cleared_by_upload(P):
+    """a list overflow is reported by every synchronising call (not only sph_sync) and a corrected
+    upload clears it."""
+    w = CASES["blob3d"]()
+    ctx = make_ctx(P, w, max_neighbours=8)
+    ctx.evaluate()
+    for call in (ctx.get_counters, ctx.timestep, ctx.sync):
+        with pytest.raises(P.SphError) as e:
+            call()
+        assert e.value.code == P.SPH_ERR_NEIGHBOUR_OVERFLOW
+    w2 = w.copy()
+    w2.h = w.h * 0.25                                     # few partners: the lists fit now
+    ctx.upload_workload(w2)
+    ctx.evaluate()
+    ctx.sync()
+    assert ctx.download(("nb_count",))["nb_count"].max() <= 8
+    o = orc.evaluate(w2, mode="brute")
+    check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    ctx.close()
+
+
+def test_timestep_without_gravity_and_with_nan(P):
+    """without SPH_F_GRAVITY the acceleration of eq. 54 is the SPH part alone also when the stages are
+    called one by one (no walk ever filled ag); a NaN in the state gives the limit 0 and a rejected RK3 step."""
+    w = CASES["C4-twin"]()
+    a = make_ctx(P, w)
+    a.build_tree(); a.find_neighbours(); a.rhs()
+    ta = a.timestep()
+    b = make_ctx(P, w)
+    b.evaluate()
+    tb = b.timestep()
+    assert ta == tb and np.isfinite(ta["acceleration"]) and ta["acceleration"] > 0
+    o = orc.evaluate(w, mode="brute")
+    assert ta["acceleration"] == pytest.approx(orc.timestep(w, o)["acceleration"], rel=1e-9)
+    a.close(); b.close()
+    w2 = w.copy()
+    w2.u[5] = np.nan
+    w2.flags |= P.SPH_F_RK3
+    c = make_ctx(P, w2)
+    c.evaluate()
+    assert c.timestep()["dt_max"] == 0.0
+    err, dt_new, ok = c.step_rk3(w.dt, 1e30)
+    assert not ok and np.isinf(err) and dt_new == 0.0
+    c.close()

@@ -38,7 +38,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(P.Material) == 8 + 15 * 8
     assert C.sizeof(P.Config) == 32 + 16 + 80
     assert C.sizeof(P.binding.StateIn) == 8 * (3 + 3 + 3 + 6 + 2 + 2 + 2)
-    assert C.sizeof(P.binding.StateOut) == 8 * (3 + 3 + 2 + 6 + 2 + 1 + 3 + 1 + 6 + 1 + 3 + 3 + 3 + 3)
+    assert C.sizeof(P.binding.StateOut) == 8 * (3 + 3 + 2 + 6 + 2 + 1 + 3 + 1 + 6 + 1 + 3 + 3 + 3 + 3 + 9 + 9)
 
 
 def test_workspace_sizing_and_config_validation(lib):
