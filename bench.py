@@ -11,7 +11,12 @@ list of PAPER.md:693) and two updates.  metric = particle-updates/s = N * RHS ev
   e2e           the same step through the C ABI with HOST buffers: sph_upload (pinned host state) ->
                 sph_step -> sph_download (host state) inside the timed region
   roofline      dominant kernel of the step, timed live by the library's CUDA-event stage brackets
-  cpu_baseline  the CPU oracle (oracle/, tree mode, as it stands) on a bounded sample, rank 0, N=1
+  cpu_baseline  the CPU oracle (oracle/, tree mode, as it stands) on a bounded sample, rank 0, N=1: on all host
+                cores and (value_1core) on one core, the paper's own comparison
+  workloads     the other BASELINE.json configs (C1-C4) measured in the same process: value, ms per step,
+                dominant stage and its roofline fraction
+  config.ms_per_step_twin   the headline workload again on its parity twin state (same geometry, perturbed
+                state: the viscosity branch and the principal-stress iteration of the pair kernel run)
   --impl reference   the oracle alone, same metric/config (there is no upstream code: PAPER.md only)
 
 Multi-GPU: the path is single-GPU by north_star ("one GPU only"); --gpus N runs N independent
@@ -39,9 +44,11 @@ METRIC = "particle-updates/s (full FP64 SPH RHS incl. tree gravity); % FP64/HBM 
 UNIT = "particle-updates/s"
 DEFAULT_WORKLOAD = "C5"
 L2_BYTES = 126 << 20
-# algorithmic FP64 flop per unit (DESIGN.md "Measurement": add = mul = cmp = 1, fma = 2, div = sqrt = 1)
-FLOP_PER_INTERACTION = 20.0     # eq. 51: 3 sub, 5 for r^2, +eps^2, sqrt, mul, div, 3 fma (6), G*M
-FLOP_PER_OPENING_TEST = 11.0    # eq. 50: 3 sub, 5 for r^2, theta^2 * r^2, compare, (s^2 precomputed)
+# algorithmic FP64 flop per unit (SURVEY.md 8(d); DESIGN.md section 5: add = mul = cmp = 1, fma = 2, div = sqrt = 1)
+FLOP_PER_INTERACTION = 20.0     # eq. 51 per ACCEPTED pseudo-particle or particle: 3 sub, 5 for r^2, +eps^2, rsqrt, cube (2),
+                                # G*M, 3 fma (6) -- the distance of an accepted cell is in here, not in the test
+FLOP_PER_OPENED_CELL = 9.0      # eq. 50 for a cell that is OPENED: 3 sub, 5 for r^2, compare (no force follows)
+FLOP_PER_VISIT_SURVEY = 3.0     # SURVEY.md 8(d) as written: "20 flop x I_a + 3 x visited nodes" (reported beside it)
 FLOP_PER_PAIR = {(3, True): 130.0, (2, True): 80.0, (3, False): 60.0, (2, False): 45.0}
 
 
@@ -114,7 +121,7 @@ def stage_work(stage, w, counters, evals):
     nstate = 2 * D + 4 + (6 if solid else 0) + (1 if damage else 0)      # doubles moved by the reorder
     passes = (D * 21 + 7) // 8
     if stage == "gravity":
-        return "alu", "TFLOP/s", FLOP_PER_INTERACTION * counters["n_inter"] + FLOP_PER_OPENING_TEST * counters["n_visit"]
+        return "alu", "TFLOP/s", FLOP_PER_INTERACTION * counters["n_inter"] + FLOP_PER_OPENED_CELL * counters["n_open"]
     if stage == "pairs":
         return "alu", "TFLOP/s", FLOP_PER_PAIR[(D, solid)] * counters["n_pairs"]
     if stage == "density":
@@ -130,20 +137,12 @@ def stage_work(stage, w, counters, evals):
     return "hbm", "GB/s", float(by) * n
 
 
-def run_ours(args, rank, world):
-    import torch
-    import paper_1604_03290_b200 as P
-    from paper_1604_03290_b200 import build as sph_build
-
-    sph_build.build()                       # fails loudly if nvcc or the sources are missing: no fallback
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
-    local = int(os.environ.get("LOCAL_RANK", rank))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-
+def measure_workload(P, torch, name, args, rank, world, dev, full):
+    """Times one workload on this rank's GPU.  Region A: exactly args.steps steps as the library runs them (sph_step
+    replays its CUDA graph), CUDA events on the library's stream.  Region B: the same steps with the library's
+    per-stage CUDA-event brackets (plain launches).  full: also the twin-state timing and the end-to-end arm."""
     t_gen = time.time()
-    w = sph_inputs.make(args.workload, scale=args.scale, seed=sph_inputs_seed(args.workload) + rank)
+    w = sph_inputs.make(name, scale=args.scale, seed=sph_inputs_seed(name) + rank)
     t_gen = time.time() - t_gen
     cfg, mats = P.config_of(w)
     stream = torch.cuda.Stream(device=dev)     # a stream of our own: sph_step may capture it into a CUDA graph
@@ -179,21 +178,39 @@ def run_ours(args, rank, world):
     for _ in range(args.warmup):
         ctx.step(w.dt)                       # the second step with the same dt captures the step graph
     ctx.sync()
-    # region A: the headline time -- sph_step as the library runs it (graph replay), no brackets
     launches0 = ctx.launch_count()
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", rank)))
     sampler.start()
     ms_dev = timed_steps()
     clocks = sampler.stop()
     launches = ctx.launch_count() - launches0
-    # region B: the same steps with the library's CUDA-event brackets around every stage (plain
-    # launches: the brackets are not part of the graph) -- stage shares and the roofline kernel's time
-    ctx.timing_enable(True)
+    ctx.timing_enable(True)                  # region B: stage brackets and the walk's work counters (about 4 % of the walk)
+    ctx.counters_enable(True)
     ctx.timing_read()
     ms_bracketed = timed_steps()
     stages = ctx.timing_read()
     ctx.timing_enable(False)
     counters = ctx.get_counters()
+    ctx.counters_enable(False)
+    out = dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters,
+               clocks=clocks, l2_flush=small, ws_bytes=ws_bytes, t_gen=t_gen)
+    if not full:
+        ctx.close()
+        return out
+
+    # ---- the same geometry on its parity twin state: the data-dependent paths of the pair kernel run ----
+    wt = sph_inputs.twin_of(w, seed=sph_inputs_seed(name) + 100 + rank)
+    ctx.upload_workload(wt)
+    for _ in range(args.warmup):
+        ctx.step(w.dt)
+    ctx.sync()
+    out["ms_twin"] = timed_steps()
+    ctx.timing_enable(True)
+    ctx.timing_read()
+    timed_steps()
+    out["stages_twin"] = ctx.timing_read()
+    ctx.timing_enable(False)
+    ctx.upload_workload(w)
 
     # ---- end-to-end arm: host buffers through the C ABI every step ----
     e2e_steps = max(1, min(args.steps, 3))
@@ -222,13 +239,49 @@ def run_ours(args, rank, world):
     for _ in range(e2e_steps):
         e2e_step()
     barrier()
-    ms_e2e = (time.perf_counter() - t0) * 1e3 / e2e_steps
-
-    fp64_peak = P.sph_measure_fp64_peak()
+    out.update(ms_e2e=(time.perf_counter() - t0) * 1e3 / e2e_steps, h2d=h2d, d2h=d2h)
     ctx.close()
-    return dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters, clocks=clocks,
-                ms_e2e=ms_e2e, h2d=h2d, d2h=d2h, fp64_peak=fp64_peak, l2_flush=small, ws_bytes=ws_bytes,
-                t_gen=t_gen)
+    return out
+
+
+def stage_tables(r, evals, fp64_peak, hbm_peak):
+    """per-stage times, shares and rooflines of one measured workload (region B)"""
+    w = r["w"]
+    tot_ms = sum(v[0] for v in r["stages"].values()) or 1.0
+    stages, roofs = {}, {}
+    for name, (ms, ln) in r["stages"].items():
+        if ln == 0:
+            continue
+        bound, unit, amount = stage_work(name, w, r["counters"], evals)
+        avg_ms = ms / evals
+        ach = amount / (avg_ms * 1e-3) * (1e-12 if bound == "alu" else 1e-9)
+        peak = fp64_peak if bound == "alu" else hbm_peak
+        stages[name] = {"ms_per_eval": round(avg_ms, 4), "share": round(ms / tot_ms, 4), "launches_per_eval": ln / evals}
+        roofs[name] = {"bound": bound, "achieved": round(ach, 3), "peak": round(peak, 2), "unit": unit,
+                       "frac": round(ach / peak, 4)}
+    return stages, roofs
+
+
+def run_ours(args, rank, world):
+    import torch
+    import paper_1604_03290_b200 as P
+    from paper_1604_03290_b200 import build as sph_build
+
+    sph_build.build()                       # fails loudly if nvcc or the sources are missing: no fallback
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", rank))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    r = measure_workload(P, torch, args.workload, args, rank, world, dev, full=True)
+    r["others"] = {}
+    if world == 1 and not args.no_other_workloads and args.workload == DEFAULT_WORKLOAD and args.scale == 1.0:
+        for name in ("C1", "C2", "C3", "C4"):      # north_star: "throughput on the five synthetic workloads"
+            torch.cuda.empty_cache()
+            r["others"][name] = measure_workload(P, torch, name, args, rank, world, dev, full=False)
+    r["fp64_peak"] = P.sph_measure_fp64_peak()
+    r["copy_gbs"] = P.sph_measure_copy_bw(1 << 30)
+    return r
 
 
 def sph_inputs_seed(name):
@@ -243,7 +296,7 @@ def oracle_time(w, budget_s=20.0):
     evaluation of workload `w`.  Small workloads are evaluated whole.  Large ones on a bounded
     sample: the evaluation is run for M1 and M2 target particles (the tree and the per-particle
     pre-pass always cover all N particles), and  T(N) = T_fixed + N * t_per  is formed from the two.
-    Returns (seconds per complete evaluation, description of the sample)."""
+    Returns (seconds per complete evaluation, description of the sample, details dict)."""
     from oracle import oracle as orc
     n = w.n
     orc.lib()
@@ -251,7 +304,8 @@ def oracle_time(w, budget_s=20.0):
         t0 = time.perf_counter()
         orc.evaluate(w, mode="tree")
         t = time.perf_counter() - t0
-        return t, f"one complete RHS evaluation of all {n} particles (oracle tree mode)"
+        return t, f"one complete RHS evaluation of all {n} particles (oracle tree mode)", \
+            {"extrapolated": False, "measured_s": round(t, 3), "n_particles": n}
     rng = np.random.default_rng(12345)
     m1 = 2000
     t1s = np.sort(rng.choice(n, m1, replace=False))
@@ -272,9 +326,25 @@ def oracle_time(w, budget_s=20.0):
         T2 = time.perf_counter() - t0
     per = max((T2 - T1) / (m2 - m1), 1e-12)
     fixed = max(T1 - per * m1, 0.0)
-    return fixed + per * n, (f"rates of {m2} random target particles of the full {n}-particle workload "
-                             f"({T2:.1f} s) and of {m1} ({T1:.1f} s); tree, order and pre-pass over all "
-                             f"particles both times; T(N) = {fixed:.2f} s + N * {per * 1e6:.2f} us")
+    desc = (f"rates of {m2} random target particles of the full {n}-particle workload "
+            f"({T2:.1f} s) and of {m1} ({T1:.1f} s); tree, order and pre-pass over all "
+            f"particles both times; T(N) = {fixed:.2f} s + N * {per * 1e6:.2f} us")
+    return fixed + per * n, desc, {"extrapolated": True, "measured_s": [round(T1, 3), round(T2, 3)],
+                                   "measured_targets": [m1, m2], "n_particles": n}
+
+
+def oracle_time_one_core(name, scale, budget_s=8.0):
+    """The same measurement on ONE host core (the paper compares its GPU code with one CPU core: PAPER.md:687,
+    :705), in a child process started with OMP_NUM_THREADS=1, on a 1/8-size instance of the workload where the full
+    one would take more than ~10 minutes.  Returns a dict or None."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    cmd = [sys.executable, os.path.abspath(__file__), "--impl", "oracle-probe", "--workload", name, "--scale", str(scale),
+           "--oracle-budget", str(budget_s)]
+    try:
+        out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600)
+        return json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception as e:                                   # the baseline is context: never fail the bench line for it
+        return {"error": repr(e)[:200]}
 
 
 def host_cores():
@@ -299,7 +369,7 @@ def run_reference(args, rank, world):
     per_step = []
     sample = ""
     for k in range(args.warmup + args.steps):
-        t_eval, sample = oracle_time(w, budget_s=6.0)
+        t_eval, sample, det = oracle_time(w, budget_s=6.0)
         if k >= args.warmup:
             per_step.append(2.0 * t_eval)            # a step is two evaluations
         if sum(per_step) > 150.0:
@@ -310,7 +380,7 @@ def run_reference(args, rank, world):
             "steps": len(per_step), "warmup": args.warmup, "ms_per_step": T * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_of_workload(w, args),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": dict({"value": value, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample}, **det),
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     return line
@@ -342,16 +412,24 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "oracle-probe"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(sph_inputs.CONFIGS))
     ap.add_argument("--scale", type=float, default=1.0, help="< 1: smaller instance of the same workload (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true", help="skip the C1-C4 lines of the default run")
+    ap.add_argument("--oracle-budget", type=float, default=8.0, help=argparse.SUPPRESS)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
 
+    if args.impl == "oracle-probe":          # child of oracle_time_one_core: one timing, threads from the environment
+        w = sph_inputs.make(args.workload, scale=args.scale)
+        t_eval, sample, det = oracle_time(w, budget_s=args.oracle_budget)
+        print(json.dumps(dict({"value": w.n / t_eval, "unit": UNIT, "cores": host_cores(), "sample": sample,
+                               "scale": args.scale}, **det)), flush=True)
+        return 0
     if args.impl == "reference":
         line = run_reference(args, rank, world)
         if line is not None:
@@ -370,6 +448,7 @@ def main():
     rmax, rsum = make_reducers(world, dev)
     ms_dev, n_total = aggregate(r["ms_dev"], w.n, world, rmax, rsum)
     ms_e2e, _ = aggregate(r["ms_e2e"], w.n, world, rmax, rsum)
+    ms_twin, _ = aggregate(r["ms_twin"], w.n, world, rmax, rsum)
     launches = int(rsum(r["launches"]))
     if rank != 0:
         torch.distributed.destroy_process_group()
@@ -381,25 +460,34 @@ def main():
     hbm_peak, hbm_src = _peaks()
 
     # per-stage table and rooflines (rank 0's replica)
-    tot_ms = sum(v[0] for v in r["stages"].values()) or 1.0
-    stages, roofs = {}, {}
-    for name, (ms, ln) in r["stages"].items():
-        if ln == 0:
-            continue
-        bound, unit, amount = stage_work(name, w, r["counters"], evals)
-        calls = evals
-        avg_ms = ms / calls
-        ach = amount / (avg_ms * 1e-3) * (1e-12 if bound == "alu" else 1e-9)
-        peak = r["fp64_peak"] if bound == "alu" else hbm_peak
-        stages[name] = {"ms_per_eval": round(avg_ms, 4), "share": round(ms / tot_ms, 4), "launches_per_eval": ln / calls}
-        roofs[name] = {"bound": bound, "achieved": round(ach, 3), "peak": round(peak, 2), "unit": unit,
-                       "frac": round(ach / peak, 4)}
+    stages, roofs = stage_tables(r, evals, r["fp64_peak"], hbm_peak)
     top = max(stages, key=lambda k: stages[k]["share"])
     roofline = dict(roofs[top])
     roofline.update({"kernel": top, "traffic": TRAFFIC_NCU.get((args.workload, top)),
                      "peak_source": ("FP64 FMA micro-benchmark measured in this run (sph_measure_fp64_peak); nominal "
                                      "148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s") if roofline["bound"] == "alu"
                      else hbm_src})
+    if top == "gravity":
+        c = r["counters"]
+        t_s = stages[top]["ms_per_eval"] * 1e-3
+        roofline["accounting"] = ("20 flop per accepted interaction (eq. 51) + 9 per OPENED cell (eq. 50); the distance of an "
+                                  "accepted cell is counted once, inside the 20")
+        roofline["frac_survey_8d"] = round((FLOP_PER_INTERACTION * c["n_inter"] + FLOP_PER_VISIT_SURVEY * c["n_visit"])
+                                           / t_s * 1e-12 / r["fp64_peak"], 4)      # "20 x I + 3 x visited nodes" as written
+    # the twin state of the same geometry (stage shares of its bracketed run)
+    twin_stages = {k: round(v[0] / evals, 4) for k, v in r["stages_twin"].items() if v[1]}
+
+    others = {}
+    for name, ro in r["others"].items():
+        st_o, rf_o = stage_tables(ro, evals, r["fp64_peak"], hbm_peak)
+        top_o = max(st_o, key=lambda k: st_o[k]["share"])
+        wo = ro["w"]
+        others[name] = {"workload": wo.name, "n_particles": wo.n, "value": wo.n * evals / (ro["ms_dev"] * 1e-3), "unit": UNIT,
+                        "ms_per_step": ro["ms_dev"] / args.steps, "ms_per_step_bracketed": ro["ms_bracketed"] / args.steps,
+                        "gpu_launches": ro["launches"], "dominant_stage": top_o, "dominant_ms_per_eval": st_o[top_o]["ms_per_eval"],
+                        "dominant_share": st_o[top_o]["share"], "roofline": rf_o[top_o],
+                        "l2": "L2 flushed between timed steps" if ro["l2_flush"] else "working set larger than L2",
+                        "clocks": ro["clocks"], "stages_ms_per_eval": {k: v["ms_per_eval"] for k, v in st_o.items()}}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_dev / args.steps, "higher_is_better": True,
@@ -412,16 +500,32 @@ def main():
                 "timing": "value: K steps as the library runs them (sph_step replays its CUDA graph), CUDA events; "
                           "stages/roofline: the same K steps again with per-stage CUDA-event brackets (plain launches)",
                 "ms_per_step_bracketed": r["ms_bracketed"] / args.steps,
+                "ms_per_step_twin": ms_twin / args.steps,
+                "twin": "same geometry and flaws, perturbed state (sph_inputs.twin_of): every branch of the rate equations "
+                        "runs on every particle; value/ms_per_step above are the nominal t = 0 state of BASELINE.json",
+                "twin_stages_ms_per_eval": twin_stages,
+                "hbm_copy_gbs_this_run": round(r["copy_gbs"], 1),
                 "counters_last_eval": r["counters"]}),
             "clocks": r["clocks"],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(r["h2d"]),
                     "d2h_bytes_per_step": int(r["d2h"]), "ms_per_step": ms_e2e},
             "gpu_launches": launches,
             "roofline": roofline, "stages": stages, "rooflines_all": roofs}
+    if others:
+        line["workloads"] = others
     if world == 1 and not args.no_cpu_baseline:
-        t_eval, sample = oracle_time(w)
-        line["cpu_baseline"] = {"value": w.n / t_eval, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
-                                "sample": sample}
+        t_eval, sample, det = oracle_time(w)
+        cb = dict({"value": w.n / t_eval, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample}, **det)
+        # one core, the paper's comparison: on a 1/8-size instance (labelled) when generating and evaluating the full
+        # one on a single core would not fit the few minutes of a default run
+        sc1 = args.scale if w.n * 60e-6 < 60.0 else args.scale / 8.0     # ~60 us per particle and core
+        one = oracle_time_one_core(args.workload, sc1)
+        if one and "value" in one:
+            cb["value_1core"] = one["value"]
+            cb["one_core"] = {k: one[k] for k in ("sample", "scale", "extrapolated", "measured_s", "n_particles") if k in one}
+        elif one:
+            cb["one_core"] = one
+        line["cpu_baseline"] = cb
     print(json.dumps(line), flush=True)
     if world > 1:
         torch.distributed.destroy_process_group()

@@ -238,10 +238,13 @@ int sph_timing_enable(sph_ctx *ctx, int on);
  * stage bracket recorded since the last read into ms[SPH_T_COUNT] / launches[SPH_T_COUNT] (HOST). */
 int sph_timing_read(sph_ctx *ctx, double *ms, int64_t *launches);
 const char *sph_timing_name(int stage);
-/* Work counters of the LAST evaluation (HOST out[4]; synchronises): internal nodes; sum over
- * particles of the partner count; sum over particles of gravity interactions (accepted pseudo-
- * particles + directly summed particles, eq. 51); sum over particles of opening tests (eq. 50: accepted
- * and opened cells).  Also reports device-side failures of the evaluation. */
+/* on != 0: the gravity walk also counts its interactions and opening tests (entries [2]-[4] of sph_get_counters;
+ * about 4 % of the walk's time, so off by default; without it those entries read 0).  Drops a captured step graph. */
+int sph_counters_enable(sph_ctx *ctx, int on);
+/* Work counters of the LAST evaluation (HOST out[5]; synchronises): [0] internal nodes; [1] sum over
+ * particles of the partner count; [2] sum over particles of gravity interactions (accepted pseudo-
+ * particles + directly summed particles, eq. 51); [3] sum over particles of opening tests (eq. 50:
+ * accepted and opened cells); [4] of those, the opened cells.  Also reports device-side failures. */
 int sph_get_counters(sph_ctx *ctx, int64_t *out);
 /* Dependency-free FP64 FMA throughput of the device [TFLOP/s] (the ALU roofline denominator;
  * MEASURED_PEAKS.json has no FP64 figure). stream: cudaStream_t. Synchronises. */

@@ -89,7 +89,7 @@ def lib():
         L.orc_rhs.argtypes = [_P(Cfg), _P(Mat), _P(State)] + [C.c_void_p] * 4 + \
                              [C.c_longlong, C.c_void_p, C.c_void_p, C.c_void_p, _P(Rates)]
         L.orc_gravity_tree.argtypes = [C.c_void_p, _P(Cfg), C.c_longlong, C.c_void_p, C.c_void_p,
-                                       C.c_void_p, C.c_void_p]
+                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_gravity_direct.argtypes = [_P(Cfg), _P(State), C.c_longlong, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
@@ -294,7 +294,9 @@ def rhs(w, off, idx, targets=None, rho=None, h=None, n_act=None):
     return out
 
 
-def gravity_tree(w, tree=None, targets=None, theta=None):
+def gravity_tree(w, tree=None, targets=None, theta=None, counts=None):
+    """Barnes-Hut accelerations (3, nt), sums of |terms| and accepted interactions per target.  counts: a dict that
+    receives the per-target work counters n_test (opening tests of eq. 50) and n_open (cells opened)."""
     tree = tree or Tree(w)
     b = _Bound(w)
     if theta is not None:
@@ -302,8 +304,11 @@ def gravity_tree(w, tree=None, targets=None, theta=None):
     t = _targets(w.n, targets)
     ag, A = np.zeros((3, t.size)), np.zeros((3, t.size))
     ni = np.zeros(t.size, dtype=np.int64)
+    nt_, no_ = np.zeros(t.size, dtype=np.int64), np.zeros(t.size, dtype=np.int64)
     lib().orc_gravity_tree(tree.handle, C.byref(b.cfg), t.size, t.ctypes.data, ag.ctypes.data,
-                           A.ctypes.data, ni.ctypes.data)
+                           A.ctypes.data, ni.ctypes.data, nt_.ctypes.data, no_.ctypes.data)
+    if counts is not None:
+        counts["n_test"], counts["n_open"] = nt_, no_
     return ag, A, ni
 
 
@@ -349,8 +354,10 @@ def evaluate(w, mode="brute", targets=None, h_iters=None):
     out["rho"] = rho
     out["nb_off"], out["nb_idx"] = off, idx
     if w.flags & F_GRAVITY:
-        ag, A, ni = gravity_tree(w, tree, t)
+        cnt = {}
+        ag, A, ni = gravity_tree(w, tree, t, counts=cnt)
         out["ag"], out["A_ag"], out["n_inter"] = ag, A, ni
+        out["n_test"], out["n_open"] = cnt["n_test"], cnt["n_open"]
     else:
         out["ag"], out["A_ag"] = np.zeros((3, t.size)), np.zeros((3, t.size))
         out["n_inter"] = np.zeros(t.size, np.int64)

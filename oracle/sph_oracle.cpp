@@ -734,7 +734,7 @@ void orc_rhs(const orc_cfg *c, const orc_mat *mats, const orc_state *s, const do
 // (PAPER.md:380); force PAPER.md:376 (eq. 51) with attractive sign and Plummer softening
 // (U21).  Particles at zero distance contribute nothing (direction undefined).
 // -------------------------------------------------------------------------------------
-struct GravAcc { double a[3]; double A[3]; i64 n_inter; };
+struct GravAcc { double a[3]; double A[3]; i64 n_inter; i64 n_test, n_open; };   // n_test: opening tests (eq. 50), n_open: of those, cells opened
 
 static inline void grav_add(GravAcc &g, int D, double G, double M, const double dx[3], double r2, double eps2) {
     double r2e = r2 + eps2;
@@ -757,8 +757,9 @@ static void grav_walk(const Tree &T, const orc_cfg *c, int id, int psorted, Grav
             double r2 = dx[0] * dx[0] + dx[1] * dx[1];
             if (D == 3) r2 = r2 + dx[2] * dx[2];
             double sl = std::ldexp(T.s0, -kn.level);                      // eq. 68
+            g.n_test++;
             if (sl * sl < th2 * r2) grav_add(g, D, c->G, kn.mass, dx, r2, eps2);
-            else grav_walk(T, c, k, psorted, g);
+            else { g.n_open++; grav_walk(T, c, k, psorted, g); }
         } else {
             for (int p = nd.plo[ch]; p < nd.phi[ch]; ++p) {
                 if (p == psorted) continue;
@@ -773,14 +774,15 @@ static void grav_walk(const Tree &T, const orc_cfg *c, int id, int psorted, Grav
 }
 
 // targets are ORIGINAL indices; ag is (3, nt) row-major; A_ag likewise; n_inter per target.
+// n_test / n_open (may be NULL): opening tests evaluated and cells opened, per target (work counters only).
 void orc_gravity_tree(void *t, const orc_cfg *c, i64 nt, const i64 *targets, double *ag, double *A_ag,
-                      i64 *n_inter) {
+                      i64 *n_inter, i64 *n_test, i64 *n_open) {
     const Tree &T = *(Tree *)t;
     std::vector<int> inv(T.n);
     for (i64 i = 0; i < T.n; ++i) inv[T.perm[i]] = (int)i;
 #pragma omp parallel for schedule(dynamic, 16)
     for (i64 k = 0; k < nt; ++k) {
-        GravAcc g = {{0, 0, 0}, {0, 0, 0}, 0};
+        GravAcc g = {{0, 0, 0}, {0, 0, 0}, 0, 0, 0};
         int ps = inv[targets[k]];
         if (!T.nodes.empty()) {
             // the root itself is always opened: the particle lies inside it (s/r >= 1/sqrt(D) > theta)
@@ -798,6 +800,8 @@ void orc_gravity_tree(void *t, const orc_cfg *c, i64 nt, const i64 *targets, dou
         }
         for (int al = 0; al < 3; ++al) { ag[al * nt + k] = g.a[al]; A_ag[al * nt + k] = g.A[al]; }
         n_inter[k] = g.n_inter;
+        if (n_test) n_test[k] = g.n_test;
+        if (n_open) n_open[k] = g.n_open;
     }
 }
 

@@ -24,7 +24,7 @@ EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sp
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
-           "sph_timing_name", "sph_get_counters", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+           "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
 SPH_T_COUNT = 11
 
 _vp = C.c_void_p
@@ -103,6 +103,7 @@ def load_library():
     L.sph_timing_name.restype = C.c_char_p
     L.sph_timing_name.argtypes = [C.c_int]
     L.sph_get_counters.argtypes = [_vp, _vp]
+    L.sph_counters_enable.argtypes = [_vp, C.c_int]
     L.sph_timestep.argtypes = [_vp, _vp]
     L.sph_step_rk3.argtypes = [_vp, C.c_double, C.c_double, _vp]
     L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
@@ -320,10 +321,13 @@ class Context:
         self._check(load_library().sph_timestep(self.handle, out.ctypes.data))
         return dict(acceleration=float(out[0]), courant=float(out[1]), change=float(out[2]), dt_max=float(out[3]))
 
+    def counters_enable(self, on=True):
+        self._check(load_library().sph_counters_enable(self.handle, int(bool(on))))
+
     def get_counters(self):
-        out = np.zeros(4, np.int64)
+        out = np.zeros(5, np.int64)
         self._check(load_library().sph_get_counters(self.handle, out.ctypes.data))
-        return dict(n_nodes=int(out[0]), n_pairs=int(out[1]), n_inter=int(out[2]), n_visit=int(out[3]))
+        return dict(n_nodes=int(out[0]), n_pairs=int(out[1]), n_inter=int(out[2]), n_visit=int(out[3]), n_open=int(out[4]))
 
 
 # ---- module-level functions with the names of the C ABI ----

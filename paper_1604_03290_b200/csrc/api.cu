@@ -538,12 +538,21 @@ const char *sph_timing_name(int stage) {
     return (stage >= 0 && stage < SPH_T_COUNT) ? names[stage] : "?";
 }
 
+int sph_counters_enable(sph_ctx *ctx, int on) {
+    if (!ctx) return SPH_ERR_ARG;
+    ctx->count_work = on ? 1 : 0;
+    if (ctx->step_graph) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }   // another kernel variant
+    ctx->last_dt = ctx->graph_dt = -1.0;
+    return SPH_OK;
+}
+
 int sph_get_counters(sph_ctx *ctx, int64_t *out) {
     if (!ctx || !out) return SPH_ERR_ARG;
     DevStatus st;
     cudaMemcpyAsync(&st, ctx->d.status, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream);
     cudaStreamSynchronize(ctx->stream);
     out[0] = st.n_nodes; out[1] = (int64_t)st.n_pairs; out[2] = (int64_t)st.n_inter; out[3] = (int64_t)st.n_visit;
+    out[4] = (int64_t)st.n_open;
     return status_flags(ctx, st, "sph_get_counters");
 }
 

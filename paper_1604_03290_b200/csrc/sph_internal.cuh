@@ -24,6 +24,7 @@ struct DevStatus {
     u64 n_pairs;        // sum over particles of |N(a)|               (A5)
     u64 n_inter;        // accepted pseudo-particles + direct particles, per particle, summed (A11)
     u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
+    u64 n_open;         // of those, the cells the particle opened (did not accept), summed   (A11)
     int n_items;        // records of the partner-search stream
     int pad;
     u64 rkerr;          // bit pattern of the error estimate of eq. 63 (sph_step_rk3)
@@ -145,6 +146,7 @@ struct sph_ctx {
     size_t ws_bytes;
     int have_state, have_tree, have_lists, have_rates;
     i64 launches;
+    int count_work;             // sph_counters_enable: the gravity walk keeps its work counters
     int sort_cur;
     SphTiming *timing;          // NULL unless sph_timing_enable(ctx, 1)
     // sph_step as a CUDA graph: captured when the same dt is asked for twice in a row, replayed after

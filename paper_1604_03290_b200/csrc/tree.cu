@@ -198,7 +198,7 @@ void sph_launch_moments(sph_ctx *ctx, int hmax_only) {
 
 __global__ void k_zero_status(Dev d) {
     d.status->n_nodes = 0;
-    d.status->n_pairs = 0; d.status->n_inter = 0; d.status->n_visit = 0;
+    d.status->n_pairs = 0; d.status->n_inter = 0; d.status->n_visit = 0; d.status->n_open = 0;
 }
 
 void sph_stage_tree(sph_ctx *ctx) {

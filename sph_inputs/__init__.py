@@ -404,6 +404,22 @@ def c5_ceres_collision(seed=1608, scale=1.0, twin=False):
     return w
 
 
+def twin_of(w, seed=0):
+    """Parity twin of an already generated nominal workload: a copy with the same geometry and flaw table and the
+    seeded perturbations of _perturb (used by bench.py to time the state the kernels see in a running simulation
+    without generating the particles and flaws a second time)."""
+    q = w.copy()
+    amp = {}
+    for k, mm in enumerate(q.materials):            # velocity-noise amplitude per material (a scale, not the EoS)
+        if mm["eos"] == EOS_TILLOTSON:
+            amp[k] = math.sqrt(mm["tA"] / mm["rho0"])
+        elif mm["eos"] == EOS_MURNAGHAN:
+            amp[k] = math.sqrt(mm["K0"] / mm["rho0"])
+        else:
+            amp[k] = math.sqrt(mm["gamma"] * (mm["gamma"] - 1.0) * float(np.mean(q.u)))
+    return _perturb(q, np.random.default_rng(seed), amp)
+
+
 CONFIGS = {"C1": c1_rubber_rings, "C1x": c1x_rubber_rings_paper, "C2": c2_gas_sphere, "C3": c3_al_impact,
            "C4": c4_basalt_impact, "C5": c5_ceres_collision}
 

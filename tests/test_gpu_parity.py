@@ -31,6 +31,7 @@ def make_ctx(P, w, export=False, **kw):
     if export:                                   # keep grad v and C of the last evaluation (A8 compared directly)
         cfg.flags |= P.SPH_F_EXPORT_GRADV
     ctx = P.sph_create(cfg, mats)
+    ctx.counters_enable(True)                     # the walk's work counters are compared with the oracle's
     ctx.upload_workload(w)
     return ctx
 
@@ -184,6 +185,10 @@ def test_full_evaluation_parity_small(P, name):
     g = ctx.download(all_fields(P))
     assert np.array_equal(g["nb_count"], np.diff(o["nb_off"]))
     check_rates(w, g, o)
+    c = ctx.get_counters()                       # the units of the roofline: exact integers on both sides
+    assert c["n_pairs"] == o["nb_off"][-1]
+    if w.flags & orc.F_GRAVITY:
+        assert (c["n_inter"], c["n_visit"], c["n_open"]) == (o["n_inter"].sum(), o["n_test"].sum(), o["n_open"].sum())
     if not (w.flags & orc.F_SOLID):
         assert not g["gradv"].any() and not g["C"].any()
     # the same kernels without the export flag give the same rates bit for bit
@@ -558,10 +563,14 @@ def test_gravity_stack_bound_small_theta(P, theta):
     ctx.gravity()
     ctx.sync()                                            # raises on err_stack
     g = ctx.download(("ag",))["ag"]
-    t = np.sort(rng.choice(n, 400, replace=False))
-    ag, A, ni = orc.gravity_tree(w, targets=t)
-    assert_close("ag", g[:, t], ag, A)
+    cnt = {}
+    ag, A, ni = orc.gravity_tree(w, counts=cnt)           # all 70 k targets: a few 1e8 opening decisions
+    assert_close("ag", g, ag, A)
     assert ni.mean() > 4000                               # many more interactions than at theta = 0.5
+    # every decision equal to the oracle's, including the pairs whose distance falls within 2^-20 of a threshold
+    # (decided by the kernel's cold path on the exactly rounded r2): the work counters are exact integers
+    c = ctx.get_counters()
+    assert (c["n_inter"], c["n_visit"], c["n_open"]) == (ni.sum(), cnt["n_test"].sum(), cnt["n_open"].sum())
     ctx.close()
 
 
