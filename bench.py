@@ -19,8 +19,9 @@ list of PAPER.md:693) and two updates.  metric = particle-updates/s = N * RHS ev
                 state: the viscosity branch and the principal-stress iteration of the pair kernel run)
   --impl reference   the oracle alone, same metric/config (there is no upstream code: PAPER.md only)
 
-Multi-GPU: the path is single-GPU by north_star ("one GPU only"); --gpus N runs N independent
-replicas (replicas only, no data-path collective), weak scaling.
+Multi-GPU (--gpus N under torchrun): ONE workload sharded by Morton ranges over the N GPUs (DESIGN.md section 9:
+replicated cheap stages, partner search / pair sums / walk on the rank's slice, one NCCL all-gather of the rate
+arrays per evaluation), strong scaling; value = particles * evaluations / max over ranks of the device time.
 """
 from __future__ import annotations
 
@@ -142,13 +143,16 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     replays its CUDA graph), CUDA events on the library's stream.  Region B: the same steps with the library's
     per-stage CUDA-event brackets (plain launches).  full: also the twin-state timing and the end-to-end arm."""
     t_gen = time.time()
-    w = sph_inputs.make(name, scale=args.scale, seed=sph_inputs_seed(name) + rank)
+    w = sph_inputs.make(name, scale=args.scale, seed=sph_inputs_seed(name))     # the same particles on every rank
     t_gen = time.time() - t_gen
     cfg, mats = P.config_of(w)
     stream = torch.cuda.Stream(device=dev)     # a stream of our own: sph_step may capture it into a CUDA graph
     torch.cuda.set_stream(stream)              # torch's events, fills and copies below go to the same stream
     ctx = P.sph_create(cfg, mats, device=dev, stream=stream)
     ctx.upload_workload(w)
+    if world > 1:                              # Morton-range sharding: this rank's slice, all-gather through NCCL
+        ctx.set_partition(rank, world)
+    lo, hi, _ = P.sph_partition(w.n, world, rank)
     ws_bytes = ctx.workspace_bytes
     small = ws_bytes < 4 * L2_BYTES       # working set may sit in the 126 MB L2: flush between steps
     flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if small else None
@@ -193,13 +197,13 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     counters = ctx.get_counters()
     ctx.counters_enable(False)
     out = dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters,
-               clocks=clocks, l2_flush=small, ws_bytes=ws_bytes, t_gen=t_gen)
+               clocks=clocks, l2_flush=small, ws_bytes=ws_bytes, t_gen=t_gen, n_own=hi - lo)
     if not full:
         ctx.close()
         return out
 
     # ---- the same geometry on its parity twin state: the data-dependent paths of the pair kernel run ----
-    wt = sph_inputs.twin_of(w, seed=sph_inputs_seed(name) + 100 + rank)
+    wt = sph_inputs.twin_of(w, seed=sph_inputs_seed(name) + 100)
     ctx.upload_workload(wt)
     for _ in range(args.warmup):
         ctx.step(w.dt)
@@ -285,7 +289,7 @@ def run_ours(args, rank, world):
 
 
 def sph_inputs_seed(name):
-    return {"C1": 1604, "C1x": 1604, "C2": 1605, "C3": 1606, "C4": 1607, "C5": 1608}[name]
+    return {"C1": 1604, "C1x": 1604, "C2": 1605, "C3": 1606, "C4": 1607, "C5": 1608, "C6": 1609}[name]
 
 
 # ---------------------------------------------------------------------------------------------
@@ -446,9 +450,10 @@ def main():
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", rank)))
 
     rmax, rsum = make_reducers(world, dev)
-    ms_dev, n_total = aggregate(r["ms_dev"], w.n, world, rmax, rsum)
-    ms_e2e, _ = aggregate(r["ms_e2e"], w.n, world, rmax, rsum)
-    ms_twin, _ = aggregate(r["ms_twin"], w.n, world, rmax, rsum)
+    # every rank contributes the particles of its own slice: the sum is the workload, the time is the slowest rank's
+    ms_dev, n_total = aggregate(r["ms_dev"], r["n_own"], world, rmax, rsum)
+    ms_e2e, _ = aggregate(r["ms_e2e"], r["n_own"], world, rmax, rsum)
+    ms_twin, _ = aggregate(r["ms_twin"], r["n_own"], world, rmax, rsum)
     launches = int(rsum(r["launches"]))
     if rank != 0:
         torch.distributed.destroy_process_group()
@@ -491,9 +496,12 @@ def main():
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_dev / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak" if world == 1 else "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_of_workload(w, args, {
-                "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                "parallelism": "single GPU" if world == 1 else
+                               f"one workload sharded by Morton ranges over {world} GPUs: tree build replicated, partner search / "
+                               f"pair sums / gravity walk on the rank's slice, one NCCL all-gather of the rates per evaluation; "
+                               f"stages, roofline and counters below are rank 0's slice",
                 "l2": "L2 flushed (252 MB write) between timed steps" if r["l2_flush"]
                       else "working set larger than L2 (%.1f GB workspace)" % (r["ws_bytes"] / 1e9),
                 "particle_steps_per_s": n_total * args.steps / (ms_dev * 1e-3),

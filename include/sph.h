@@ -194,6 +194,33 @@ int sph_timestep(sph_ctx *ctx, double *out);
  * dst_is_device: 1 = DEVICE buffers (asynchronous), 0 = HOST buffers (synchronises). */
 int sph_download(sph_ctx *ctx, const sph_state_out *dst, int dst_is_device);
 
+/* ---- Morton-range sharding over the GPUs of one node (the paper: "future work") ----
+ * One process and one context per GPU; every rank uploads the SAME full state.  The cheap global stages (keys, sort,
+ * reorder, octree, pseudo-particles, pre-pass, update) run replicated on every rank; the expensive per-particle stages
+ * (partner search, pair sums, gravity walk) run only for the rank's contiguous slice of the Morton order; then ONE
+ * all-gather per evaluation completes the rate arrays on every rank (no reduction: every rate is written by exactly one
+ * rank, and a particle's arithmetic does not depend on the rank that does it, so the sharded result equals the
+ * single-GPU result bit for bit).
+ *
+ * sph_partition (host only): slice = ceil(n / world) rounded up to a multiple of 32 (warp groups never straddle two
+ * ranks); rank r owns the sorted indices [lo, hi) = [min(n, r slice), min(n, (r + 1) slice)).  Any pointer may be NULL.
+ *
+ * sph_exchange_fn: the caller's in-place all-gather, called by the library at the end of sph_evaluate (or of sph_rhs /
+ * sph_gravity when called alone) with n_arrays DEVICE arrays of world * slice_elems elements of elem_bytes[k] bytes each;
+ * rank r has filled elements [r slice_elems, (r + 1) slice_elems) of every array; on return (stream-ordered on
+ * cuda_stream) every array must be complete on every rank.  Return 0, or non-zero to fail the call with SPH_ERR_CUDA.
+ * paper_1604_03290_b200/binding.py supplies one built on torch.distributed (NCCL over NVLink).
+ *
+ * sph_set_partition: before the next evaluation; world = 1 (or fn = NULL with world = 1) switches sharding off.
+ * With SPH_F_DENSITY_SUM, or SPH_F_VARIABLE_H with h_iters > 0, the partner search and the density sum stay replicated
+ * (every particle's density and smoothing length feed its partners' sums); the pair sums and the walk are still sharded.
+ * sph_get_neighbours then returns the lists of the rank's own slice only; the work counters are per rank.  sph_step does
+ * not capture CUDA graphs while a partition is set. */
+typedef int (*sph_exchange_fn)(void *user, void *cuda_stream, int n_arrays, void *const *arrays, const int32_t *elem_bytes,
+                               int64_t slice_elems);
+int sph_partition(int64_t n, int world, int rank, int64_t *lo, int64_t *hi, int64_t *slice);
+int sph_set_partition(sph_ctx *ctx, int rank, int world, sph_exchange_fn fn, void *user);
+
 /* Wait for all enqueued work; returns the first device-side failure if any. */
 int sph_sync(sph_ctx *ctx);
 

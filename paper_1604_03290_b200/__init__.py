@@ -2,4 +2,4 @@
 C-ABI library libsph_b200.so built from csrc/*.cu.  See include/sph.h and DESIGN.md."""
 from .binding import *  # noqa: F401,F403
 from .binding import (Config, Context, Material, SphError, config_of, load_library, make_config,
-                      make_materials, EXPORTS, LIB_PATH, RATE_FIELDS, STATE_FIELDS)
+                      make_materials, EXPORTS, LIB_PATH, RATE_FIELDS, STATE_FIELDS, sph_partition, all_gather_slices)

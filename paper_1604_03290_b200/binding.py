@@ -24,8 +24,11 @@ EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sp
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
-           "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+           "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_partition", "sph_set_partition", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
 SPH_T_COUNT = 11
+
+# the caller's in-place all-gather (include/sph.h: sph_exchange_fn)
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_int32), C.c_int64)
 
 _vp = C.c_void_p
 
@@ -104,6 +107,8 @@ def load_library():
     L.sph_timing_name.argtypes = [C.c_int]
     L.sph_get_counters.argtypes = [_vp, _vp]
     L.sph_counters_enable.argtypes = [_vp, C.c_int]
+    L.sph_partition.argtypes = [C.c_int64, C.c_int, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.sph_set_partition.argtypes = [_vp, C.c_int, C.c_int, EXCHANGE_FN, _vp]
     L.sph_timestep.argtypes = [_vp, _vp]
     L.sph_step_rk3.argtypes = [_vp, C.c_double, C.c_double, _vp]
     L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
@@ -321,6 +326,34 @@ class Context:
         self._check(load_library().sph_timestep(self.handle, out.ctypes.data))
         return dict(acceleration=float(out[0]), courant=float(out[1]), change=float(out[2]), dt_max=float(out[3]))
 
+    # ---- Morton-range sharding over the GPUs of a node (include/sph.h) ----
+    def set_partition(self, rank, world, group=None, exchange=None):
+        """sph_set_partition.  Every rank must have uploaded the same full state.  The all-gather of the rate arrays
+        at the end of an evaluation is `exchange(tensors, slice_bytes)` if given (tests emulate ranks with it), else
+        all_gather_slices over the torch.distributed group (NCCL: one in-place all-gather per array over NVLink)."""
+        torch = self.torch
+        if world <= 1:
+            self._check(load_library().sph_set_partition(self.handle, 0, 1, EXCHANGE_FN(0), None))
+            self._xfn = None
+            return
+
+        def hook(_user, _stream, n_arrays, arrays, elem_bytes, slice_elems):
+            try:
+                with torch.cuda.stream(self.stream):
+                    sb = [int(elem_bytes[k]) * int(slice_elems) for k in range(n_arrays)]
+                    ts = [device_bytes(torch, int(arrays[k]), world * sb[k], self.device) for k in range(n_arrays)]
+                    if exchange is not None:
+                        exchange(ts, sb)
+                    else:
+                        all_gather_slices(ts, sb, rank, group)
+                return 0
+            except Exception as e:                        # never let an exception cross the C boundary
+                self._xerr = e
+                return 1
+
+        self._xfn = EXCHANGE_FN(hook)                     # keep the callback object alive
+        self._check(load_library().sph_set_partition(self.handle, int(rank), int(world), self._xfn, None))
+
     def counters_enable(self, on=True):
         self._check(load_library().sph_counters_enable(self.handle, int(bool(on))))
 
@@ -328,6 +361,36 @@ class Context:
         out = np.zeros(5, np.int64)
         self._check(load_library().sph_get_counters(self.handle, out.ctypes.data))
         return dict(n_nodes=int(out[0]), n_pairs=int(out[1]), n_inter=int(out[2]), n_visit=int(out[3]), n_open=int(out[4]))
+
+
+def sph_partition(n, world, rank):
+    """(lo, hi, slice) of sph_partition: the sorted indices rank `rank` of `world` owns and the slice length."""
+    lo, hi, sl = C.c_int64(), C.c_int64(), C.c_int64()
+    rc = load_library().sph_partition(int(n), int(world), int(rank), C.byref(lo), C.byref(hi), C.byref(sl))
+    if rc != SPH_OK:
+        raise SphError(rc, "sph_partition")
+    return lo.value, hi.value, sl.value
+
+
+class _DeviceBytes:
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def device_bytes(torch, ptr, nbytes, device):
+    """a uint8 torch tensor over `nbytes` of device memory at `ptr` (no copy; the library owns the memory)"""
+    return torch.as_tensor(_DeviceBytes(ptr, nbytes), device=device)
+
+
+def all_gather_slices(tensors, slice_bytes, rank, group=None):
+    """In-place all-gather of flat byte tensors: rank r has filled bytes [r sb, (r + 1) sb) of every tensor; afterwards
+    every tensor is complete on every rank.  Works on CUDA tensors (NCCL) and on CPU tensors (gloo, used by the tests)."""
+    import torch.distributed as dist
+    for t, sb in zip(tensors, slice_bytes):
+        own = t[rank * sb:(rank + 1) * sb]
+        if not t.is_cuda:
+            own = own.clone()                             # gloo: no aliasing of input and output
+        dist.all_gather_into_tensor(t, own, group=group)
 
 
 # ---- module-level functions with the names of the C ABI ----

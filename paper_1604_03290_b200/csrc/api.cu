@@ -100,15 +100,16 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.bmark = b.take<u64>(n + 1); z.bscan = b.take<u64>(n + 1);
     z.scan_tmp = b.take<u64>(sph_scan_scratch_elems((i64)n + 1) + 2);
     z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);
-    z.nb_cnt = b.take<int>(n); z.own_cnt = b.take<int>(n);
+    const size_t np_ = n + SPH_RATE_PAD;                 // arrays the ranks exchange: world * slice <= n + 32 * world elements
+    z.nb_cnt = b.take<int>(np_); z.own_cnt = b.take<int>(n);
     z.p = b.take<double>(n); z.cs = b.take<double>(n);
     z.prec = b.take<double>(n * PR_REC);
-    z.drho = b.take<double>(n); z.du = b.take<double>(n); z.ddmg = b.take<double>(n); z.strain = b.take<double>(n);
-    for (int a = 0; a < 3; ++a) { z.dv[a] = b.take<double>(n); z.ag[a] = b.take<double>(n); }
-    for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(n);
-    z.n_act_new = b.take<int>(n);
-    for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? n : 1);
-    for (int k = 0; k < 9; ++k) { z.gradv[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? n : 1); z.Cten[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? n : 1); }
+    z.drho = b.take<double>(np_); z.du = b.take<double>(np_); z.ddmg = b.take<double>(np_); z.strain = b.take<double>(np_);
+    for (int a = 0; a < 3; ++a) { z.dv[a] = b.take<double>(np_); z.ag[a] = b.take<double>(np_); }
+    for (int k = 0; k < 6; ++k) z.dS[k] = b.take<double>(np_);
+    z.n_act_new = b.take<int>(np_);
+    for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? np_ : 1);
+    for (int k = 0; k < 9; ++k) { z.gradv[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); z.Cten[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); }
     z.stage = b.take<double>(n);
     z.stage_i = b.take<int>(n);
     Mats *md = b.take<Mats>(1);
@@ -469,6 +470,8 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     Dev &d = c->d;
     d.D = cfg->dim; d.L = cfg_L(cfg); d.flags = cfg->flags; d.cap = cfg_cap(cfg);
     d.n = (int)cfg->n; d.n_des = cfg->n_des;
+    d.r_lo = 0; d.r_hi = d.n;
+    c->rank = 0; c->world = 1; c->slice = cfg->n; c->xfn = nullptr; c->xuser = nullptr; c->in_evaluate = 0;
     d.theta2 = cfg->theta * cfg->theta;
     d.G = cfg->G;
     d.eps2 = cfg->eps_soft * cfg->eps_soft;
@@ -624,6 +627,59 @@ int sph_timestep(sph_ctx *ctx, double *out) {
     return status_flags(ctx, st, "sph_timestep");
 }
 
+// ------------------------------------------------------------------------------------------------
+// Morton-range sharding (include/sph.h): partition and the one all-gather per evaluation
+// ------------------------------------------------------------------------------------------------
+int sph_partition(int64_t n, int world, int rank, int64_t *lo, int64_t *hi, int64_t *slice) {
+    if (n < 1 || world < 1 || world > SPH_MAX_WORLD || rank < 0 || rank >= world) return SPH_ERR_ARG;
+    const int64_t per = (n + world - 1) / world;
+    const int64_t sl = (per + 31) / 32 * 32;
+    const int64_t l = std::min<int64_t>(n, (int64_t)rank * sl), h = std::min<int64_t>(n, l + sl);
+    if (lo) *lo = l;
+    if (hi) *hi = h;
+    if (slice) *slice = sl;
+    return SPH_OK;
+}
+
+int sph_set_partition(sph_ctx *ctx, int rank, int world, sph_exchange_fn fn, void *user) {
+    if (!ctx) return SPH_ERR_ARG;
+    int64_t lo, hi, sl;
+    if (sph_partition(ctx->d.n, world, rank, &lo, &hi, &sl) != SPH_OK) return fail(ctx, SPH_ERR_ARG, "sph_set_partition: bad rank / world");
+    if (world > 1 && !fn) return fail(ctx, SPH_ERR_ARG, "sph_set_partition: world > 1 needs an exchange function");
+    ctx->rank = rank; ctx->world = world; ctx->slice = sl;
+    ctx->xfn = (world > 1) ? fn : nullptr; ctx->xuser = user;
+    ctx->d.r_lo = (int)lo; ctx->d.r_hi = (int)hi;
+    ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
+    if (ctx->step_graph) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }
+    ctx->last_dt = ctx->graph_dt = -1.0;
+    return SPH_OK;
+}
+
+// which: 1 = the arrays sph_rhs fills, 2 = the gravitational acceleration, 3 = both
+static int exchange_rates(sph_ctx *ctx, int which) {
+    if (ctx->world <= 1 || !ctx->xfn) return SPH_OK;
+    Dev &d = ctx->d;
+    void *arr[64];
+    int32_t eb[64];
+    int na = 0;
+    auto add = [&](void *p, int bytes) { arr[na] = p; eb[na] = bytes; ++na; };
+    if (which & 1) {
+        add(d.drho, 8); add(d.du, 8);
+        // all components, also the zero rows of a 2-D run: every array a download can return is complete on every rank
+        for (int a = 0; a < 3; ++a) add(d.dv[a], 8);
+        if (d.flags & SPH_F_SOLID) for (int k = 0; k < 6; ++k) add(d.dS[k], 8);
+        if (d.flags & SPH_F_DAMAGE) { add(d.ddmg, 8); add(d.strain, 8); add(d.n_act_new, 4); }
+        if (d.flags & SPH_F_XSPH) for (int a = 0; a < 3; ++a) add(d.dxs[a], 8);
+        if ((d.flags & SPH_F_SOLID) && (d.flags & SPH_F_EXPORT_GRADV)) for (int k = 0; k < 9; ++k) { add(d.gradv[k], 8); add(d.Cten[k], 8); }
+        add(d.nb_cnt, 4);
+    }
+    if ((which & 2) && (d.flags & SPH_F_GRAVITY)) for (int a = 0; a < 3; ++a) add(d.ag[a], 8);
+    if (na == 0) return SPH_OK;
+    if (ctx->xfn(ctx->xuser, (void *)ctx->stream, na, arr, eb, (int64_t)ctx->slice) != 0)
+        return fail(ctx, SPH_ERR_CUDA, "the caller's exchange function (all-gather of the rates) failed");
+    return SPH_OK;
+}
+
 int sph_upload(sph_ctx *ctx, const sph_state_in *s, int src_is_device) {
     if (!ctx || !s) return SPH_ERR_ARG;
     Dev &d = ctx->d;
@@ -668,6 +724,7 @@ int sph_rhs(sph_ctx *ctx) {
     if (!ctx->have_tree || !ctx->have_lists) return fail(ctx, SPH_ERR_STATE, "sph_rhs before sph_find_neighbours");
     sph_stage_rhs(ctx);
     ctx->have_rates |= 1;
+    if (!ctx->in_evaluate) { const int rc = exchange_rates(ctx, 1); if (rc != SPH_OK) return rc; }
     return check_cuda(ctx, "sph_rhs");
 }
 
@@ -676,22 +733,31 @@ int sph_gravity(sph_ctx *ctx) {
     if (!ctx->have_tree) return fail(ctx, SPH_ERR_STATE, "sph_gravity before sph_build_tree");
     sph_stage_gravity(ctx);
     ctx->have_rates |= 2;
+    if (!ctx->in_evaluate) { const int rc = exchange_rates(ctx, 2); if (rc != SPH_OK) return rc; }
     return check_cuda(ctx, "sph_gravity");
 }
 
 int sph_evaluate(sph_ctx *ctx) {
+    if (!ctx) return SPH_ERR_ARG;
     int rc;
     if ((rc = sph_build_tree(ctx)) != SPH_OK) return rc;
     if ((rc = sph_find_neighbours(ctx)) != SPH_OK) return rc;
-    if ((rc = sph_rhs(ctx)) != SPH_OK) return rc;
-    if (ctx->grav_reuse) {                   // decoupled step: the stored field, brought into the new order
-        StageTimer tm(ctx, SPH_T_GRAVITY);
-        k_ag_take<<<sph_ceil_div(ctx->d.n, 256), 256, 0, ctx->stream>>>(ctx->d);
-        ctx->launches += 1;
-        ctx->have_rates |= 2;
-        return check_cuda(ctx, "sph_evaluate");
+    ctx->in_evaluate = 1;                    // sharded: ONE all-gather for the whole evaluation, after the walk
+    rc = sph_rhs(ctx);
+    if (rc == SPH_OK) {
+        if (ctx->grav_reuse) {               // decoupled step: the stored field (complete on every rank), brought into the new order
+            StageTimer tm(ctx, SPH_T_GRAVITY);
+            k_ag_take<<<sph_ceil_div(ctx->d.n, 256), 256, 0, ctx->stream>>>(ctx->d);
+            ctx->launches += 1;
+            ctx->have_rates |= 2;
+        } else {
+            rc = sph_gravity(ctx);
+        }
     }
-    return sph_gravity(ctx);
+    ctx->in_evaluate = 0;
+    if (rc != SPH_OK) return rc;
+    if ((rc = exchange_rates(ctx, ctx->grav_reuse ? 1 : 3)) != SPH_OK) return rc;
+    return check_cuda(ctx, "sph_evaluate");
 }
 
 // the launches of one predictor-corrector step, enqueued on ctx->stream
@@ -735,7 +801,7 @@ static int step_enqueue(sph_ctx *ctx, double dt) {
 int sph_step(sph_ctx *ctx, double dt) {
     if (!ctx) return SPH_ERR_ARG;
     if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
-    if (ctx->timing || ctx->graphs_off || ctx->cfg.gravity_every > 1) return step_enqueue(ctx, dt);
+    if (ctx->timing || ctx->graphs_off || ctx->cfg.gravity_every > 1 || ctx->world > 1) return step_enqueue(ctx, dt);
     if (ctx->step_graph && ctx->graph_dt == dt) {
         if (cudaGraphLaunch(ctx->step_graph, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
         ctx->launches += ctx->graph_launches;
@@ -958,7 +1024,10 @@ int sph_get_neighbours(sph_ctx *ctx, int64_t *off, int32_t *idx, int64_t cap) {
     off[0] = 0;
     {
         std::vector<int> co(n);
-        for (size_t i = 0; i < n; ++i) co[(size_t)perm[i]] = cnt[i];
+        for (size_t i = 0; i < n; ++i) {       // sharded: only the rank's own slice has lists (the counts are complete)
+            if ((int)i < d.r_lo || (int)i >= d.r_hi) cnt[i] = 0;
+            co[(size_t)perm[i]] = cnt[i];
+        }
         for (size_t o = 0; o < n; ++o) off[o + 1] = off[o] + co[o];
     }
     if (!idx) return SPH_OK;

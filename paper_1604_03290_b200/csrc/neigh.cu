@@ -148,11 +148,11 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     __shared__ double s_c[NB_WARPS][4][32];
 
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int g = blockIdx.x * NB_WARPS + w;
+    const int g = d.r_lo / 32 + blockIdx.x * NB_WARPS + w;   // groups of the rank's slice [r_lo, r_hi) (all of them on one GPU)
     const int n = d.n;
-    if (g * 32 >= n) return;
+    if (g * 32 >= d.r_hi) return;
     const int i = g * 32 + lane;
-    const bool valid = i < n;
+    const bool valid = i < d.r_hi;
     const int ii = valid ? i : n - 1;
     const unsigned FULL = 0xffffffffu;
 
@@ -250,10 +250,18 @@ __global__ void k_writeback_h(Dev d) {
     d.h[d.perm[i]] = d.sh[i];
 }
 
+// With a partition set (sph_set_partition) the walk covers the rank's slice only -- unless every particle's list is
+// needed on every rank: the density sum (eq. 28) and the eq.-73 update feed the partners' sums.
+static bool lists_replicated(const sph_ctx *ctx) {
+    return (ctx->d.flags & SPH_F_DENSITY_SUM) || ((ctx->d.flags & SPH_F_VARIABLE_H) && ctx->cfg.h_iters > 0);
+}
+
 template <int D>
 static void launch_neigh(sph_ctx *ctx, bool varh, bool count_only) {
-    Dev &d = ctx->d;
-    const int groups = sph_ceil_div(d.n, 32);
+    Dev d = ctx->d;
+    if (lists_replicated(ctx)) { d.r_lo = 0; d.r_hi = d.n; }
+    const int groups = sph_ceil_div(d.r_hi - d.r_lo, 32);
+    if (groups == 0) return;
     const int blocks = sph_ceil_div(groups, NB_WARPS);
     if (count_only) k_neigh<D, false, true><<<blocks, NB_WARPS * 32, 0, ctx->stream>>>(d);
     else if (varh) k_neigh<D, true, false><<<blocks, NB_WARPS * 32, 0, ctx->stream>>>(d);

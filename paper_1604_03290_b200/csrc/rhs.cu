@@ -93,11 +93,11 @@ template <> struct KNorm<3> { static constexpr double s = 8.0 / 3.14159265358979
 
 template <int D, bool VARH>
 __global__ void __launch_bounds__(128) k_density(Dev d) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = d.r_lo + blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const int g = i >> 5;
-    if (g * 32 >= d.n) return;
-    const bool valid = i < d.n;
+    if (g * 32 >= d.r_hi) return;
+    const bool valid = i < d.r_hi;
     const int ii = valid ? i : d.n - 1;
     const double xi = d.sx[0][ii], yi = d.sx[1][ii], zi = (D == 3) ? d.sx[2][ii] : 0.0, Hi = d.sh[ii];
     const int cnt = valid ? d.nb_cnt[ii] : 0;
@@ -204,10 +204,10 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
     constexpr int SI[6] = {0, 1, (D == 3) ? 2 : 3, 3, 4, 5};   // 2-D: xx xy yy -> 0 1 3
     __shared__ __align__(16) double s_buf[PR_WARPS][2][32 * PR_STRIDE];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int g = blockIdx.x * PR_WARPS + w;
-    if (g * 32 >= d.n) return;
+    const int g = d.r_lo / 32 + blockIdx.x * PR_WARPS + w;   // groups of the rank's slice (all of them on one GPU)
+    if (g * 32 >= d.r_hi) return;
     const int i = g * 32 + lane;
-    const bool valid = i < d.n;
+    const bool valid = i < d.r_hi;
     const int ii = valid ? i : d.n - 1;
     const unsigned FULL = 0xffffffffu;
     const double *__restrict__ prec = d.prec;
@@ -427,9 +427,14 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_materi
                 const double K = (mt.eos == SPH_EOS_TILLOTSON) ? mt.tA : mt.K0;
                 const double E = 9.0 * K * mt.mu / (3.0 * K + mt.mu);
                 strain = smax / ((1.0 - dd) * E);
-                int c = 0;
-                for (i64 j = f0; j < f1; ++j) c += (d.flaw_eps[j] <= strain) ? 1 : 0;
-                nact = max(nact, c);
+                // thresholds are ascending per particle (sph.h, eq. 45): the number of activated flaws is the
+                // position of the first threshold above the strain (bisection: ~4 reads instead of ~15)
+                i64 lo = f0, hi = f1;
+                while (lo < hi) {
+                    const i64 mid = (lo + hi) >> 1;
+                    if (d.flaw_eps[mid] <= strain) lo = mid + 1; else hi = mid;
+                }
+                nact = max(nact, (int)(lo - f0));
                 const double cg = 0.4 * sqrt((K + 4.0 / 3.0 * (1.0 - dd) * mt.mu) / rhoi);
                 if (dd < (double)nact / (double)ntot) ddmg = (double)nact * cg / Hi;
             }
@@ -446,11 +451,13 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
     const int n = d.n;
     const bool varh = (d.flags & SPH_F_VARIABLE_H) != 0, solid = (d.flags & SPH_F_SOLID) != 0;
     const int gb = sph_ceil_div((i64)sph_ceil_div(n, 32) * 32, 128);
-    const int pb = sph_ceil_div(sph_ceil_div(n, 32), PR_WARPS);
+    const int pb = sph_ceil_div(sph_ceil_div(d.r_hi - d.r_lo, 32), PR_WARPS);   // pair sums: the rank's slice
     if (d.flags & SPH_F_DENSITY_SUM) {
         StageTimer tm(ctx, SPH_T_DENSITY);
-        if (varh) k_density<D, true><<<gb, 128, 0, ctx->stream>>>(d);
-        else k_density<D, false><<<gb, 128, 0, ctx->stream>>>(d);
+        Dev dd = d;                              // every particle's density on every rank (its partners read it)
+        dd.r_lo = 0; dd.r_hi = n;
+        if (varh) k_density<D, true><<<gb, 128, 0, ctx->stream>>>(dd);
+        else k_density<D, false><<<gb, 128, 0, ctx->stream>>>(dd);
         ctx->launches += 1;
     }
     {
@@ -461,6 +468,7 @@ static void rhs_dim(sph_ctx *ctx, const sph_material *mats) {
     StageTimer tm(ctx, SPH_T_PAIRS);
     const bool extra = (d.flags & (SPH_F_ART_STRESS | SPH_F_XSPH)) != 0;
 #define SPH_PAIRS(S, V, E) k_pairs<D, S, V, E><<<pb, PR_WARPS * 32, 0, ctx->stream>>>(d, mats)
+    if (pb == 0) return;                         // a rank without particles (more ranks than slices)
     if (solid) {
         if (varh) { if (extra) SPH_PAIRS(true, true, true); else SPH_PAIRS(true, true, false); }
         else { if (extra) SPH_PAIRS(true, false, true); else SPH_PAIRS(true, false, false); }

@@ -12,6 +12,8 @@ typedef long long i64;
 
 
 #define SPH_MAX_MAT 16
+#define SPH_MAX_WORLD 64
+#define SPH_RATE_PAD (32 * SPH_MAX_WORLD)   // rate arrays are world * slice <= n + 32 * world long (sph_set_partition)
 #define SPH_WARP 32
 
 // Device-side status block (one per context, in the workspace).
@@ -76,6 +78,7 @@ struct Dev {
     int D, L, flags, cap;       // cap = max_neighbours
     int n;
     int n_des;
+    int r_lo, r_hi;             // sorted range whose partner lists, pair sums and walks THIS rank computes (0, n on one GPU)
     double theta2, G, eps2, av_alpha, av_beta, av_eps;
     double as_eps, as_n, as_mpd, xsph;
     // ---- master state, original order ----
@@ -147,6 +150,13 @@ struct sph_ctx {
     int have_state, have_tree, have_lists, have_rates;
     i64 launches;
     int count_work;             // sph_counters_enable: the gravity walk keeps its work counters
+    // Morton-range sharding over the GPUs of a node (sph_set_partition): rank, ranks, slice length, the caller's
+    // all-gather, and whether an evaluation is collecting its arrays for ONE exchange at its end
+    int rank, world;
+    i64 slice;
+    sph_exchange_fn xfn;
+    void *xuser;
+    int in_evaluate;
     int sort_cur;
     SphTiming *timing;          // NULL unless sph_timing_enable(ctx, 1)
     // sph_step as a CUDA graph: captured when the same dt is asked for twice in a row, replayed after

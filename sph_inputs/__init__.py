@@ -404,6 +404,69 @@ def c5_ceres_collision(seed=1608, scale=1.0, twin=False):
     return w
 
 
+# Table 1 of the paper (Benz & Asphaug 1999): basalt and water ice; Table 2 (the two k
+# values printed on one line: basalt 1e61 m^-3 with m = 16, ice 1e46 m^-3 with m = 9.1)
+BASALT_T1 = material(EOS_TILLOTSON, rho0=2700.0, tA=26.7e9, tB=26.7e9, tE0=487e6, tEiv=4.72e6, tEcv=18.2e6, ta=0.5,
+                     tb=1.5, talpha=5.0, tbeta=5.0, mu=22.7e9, Y0=3.5e9, brittle=1)
+ICE = material(EOS_TILLOTSON, rho0=917.0, tA=9.47e9, tB=9.47e9, tE0=10e6, tEiv=0.773e6, tEcv=3.04e6, ta=0.3, tb=0.1,
+               talpha=10.0, tbeta=5.0, mu=2.8e9, Y0=1e9, brittle=1)
+WEIBULL_T2 = {0: (1e61, 16.0), 1: (1e46, 9.1)}      # material index -> (k [m^-3], m)
+
+
+# C6 (second workload): the two-material bodies of the paper's section 5.1:
+# a target of one Ceres mass with a basalt core and a 30 wt-% water-ice mantle (R_T = 509 km) and a solid-basalt
+# projectile of the same mass (R_P = 437 km), in contact at 45 degrees like C5, both brittle with their own Weibull sets.
+def c6_ice_mantle(seed=1609, scale=1.0, twin=False):
+    rng = np.random.default_rng(seed)
+    M = 9.43e20
+    v_core, v_ice = 0.7 * M / BASALT_T1["rho0"], 0.3 * M / ICE["rho0"]
+    r_core = (3.0 * v_core / (4.0 * math.pi)) ** (1.0 / 3.0)
+    r_t = (3.0 * (v_core + v_ice) / (4.0 * math.pi)) ** (1.0 / 3.0)            # 509 km
+    r_p = (3.0 * (M / BASALT_T1["rho0"]) / (4.0 * math.pi)) ** (1.0 / 3.0)      # 437 km
+    n_tot = 400_000.0 * scale                                                    # twice the paper's 200 000
+    dx = ((4.0 / 3.0) * math.pi * (r_t ** 3 + r_p ** 3) / n_tot) ** (1.0 / 3.0)
+    tgt, prj = _lattice_in_sphere(dx, r_t), _lattice_in_sphere(dx, r_p)
+    nt, npj = tgt.shape[1], prj.shape[1]
+    n = nt + npj
+    mat = np.zeros(n, dtype=np.int32)
+    mat[:nt] = (np.sqrt((tgt ** 2).sum(0)) > r_core).astype(np.int32)           # 1 = ice mantle
+    sep = r_t + r_p + dx
+    c = sep * np.array([math.cos(math.pi / 4), math.sin(math.pi / 4), 0.0])
+    frac = r_p ** 3 / (r_t ** 3 + r_p ** 3)                                       # place the contact point near the origin
+    x = np.concatenate([tgt - frac * c[:, None], prj + (1.0 - frac) * c[:, None]], axis=1)
+    x += rng.uniform(-0.01 * dx, 0.01 * dx, (3, n))
+    x = np.ascontiguousarray(x)
+    mats = [BASALT_T1, ICE]
+    rho = np.array([m_["rho0"] for m_ in mats])[mat]
+    st = _zeros_state(n)
+    v_imp = 877.0                                                                # 1.7 v_esc
+    st["v"][0, :nt] = +0.5 * v_imp
+    st["v"][0, nt:] = -0.5 * v_imp
+    # flaws: every material with its own Weibull set over its own volume (eq. 45 per material)
+    cnt = np.zeros(n, dtype=np.int64)
+    parts = {}
+    for k, (k_w, m_w) in WEIBULL_T2.items():
+        idx = np.flatnonzero(mat == k)
+        vol = idx.size * dx ** 3
+        off_k, eps_k = weibull_flaws(rng, idx, n, k_w, m_w, vol)
+        cnt += off_k[1:] - off_k[:-1]
+        parts[k] = eps_k
+    off = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(cnt, out=off[1:])
+    eps = np.empty(int(off[-1]), dtype=np.float64)
+    owner = np.repeat(mat, cnt)                                                  # material of every CSR slot
+    for k in parts:
+        eps[owner == k] = parts[k]
+    w = Workload(name="C6-ice-mantle-collision-gravity", dim=3,
+                 flags=F_SOLID | F_PLASTIC | F_DAMAGE | F_GRAVITY, materials=mats, x=x, m=rho * dx ** 3, rho=rho,
+                 h=np.full(n, 2.6 * dx), mat=mat, flaw_off=off, flaw_eps=eps, theta=0.5, G=6.674e-11, eps_soft=0.0,
+                 av_alpha=0.5, av_beta=0.0, dt=0.05, steps=5, max_neighbours=128,
+                 meta=dict(dx=dx, n_target=nt, n_projectile=npj, r_core=r_core, r_target=r_t, r_projectile=r_p), **st)
+    if twin:
+        _perturb(w, rng, {k: math.sqrt(mm["tA"] / mm["rho0"]) for k, mm in enumerate(mats)})
+    return w
+
+
 def twin_of(w, seed=0):
     """Parity twin of an already generated nominal workload: a copy with the same geometry and flaw table and the
     seeded perturbations of _perturb (used by bench.py to time the state the kernels see in a running simulation
@@ -421,7 +484,7 @@ def twin_of(w, seed=0):
 
 
 CONFIGS = {"C1": c1_rubber_rings, "C1x": c1x_rubber_rings_paper, "C2": c2_gas_sphere, "C3": c3_al_impact,
-           "C4": c4_basalt_impact, "C5": c5_ceres_collision}
+           "C4": c4_basalt_impact, "C5": c5_ceres_collision, "C6": c6_ice_mantle}
 
 
 def make(name, scale=1.0, twin=False, seed=None):

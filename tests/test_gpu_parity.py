@@ -165,6 +165,7 @@ CASES = {
     "C3-twin": lambda: sph_inputs.make("C3", scale=0.006, twin=True),
     "C4-twin": lambda: sph_inputs.make("C4", scale=0.002, twin=True),
     "C5-twin": lambda: sph_inputs.make("C5", scale=0.001, twin=True),
+    "C6-twin": lambda: sph_inputs.make("C6", scale=0.006, twin=True),      # two brittle materials, two Weibull sets
     "blob3d": lambda: sph_inputs.random_blob(2500, dim=3, seed=3, duplicates=7),
     "blob2d": lambda: sph_inputs.random_blob(1500, dim=2, seed=4, duplicates=5),
     "blob3d-varh": lambda: sph_inputs.random_blob(2000, dim=3, seed=5, variable_h=True),
@@ -641,3 +642,105 @@ def test_timestep_without_gravity_and_with_nan(P):
     err, dt_new, ok = c.step_rk3(w.dt, 1e30)
     assert not ok and np.isinf(err) and dt_new == 0.0
     c.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Morton-range sharding: W virtual ranks on ONE GPU, one context and one host thread
+# each.  The all-gather the library asks for at the end of every evaluation is emulated on the host side: a thread
+# synchronises its own stream, waits at a barrier for the others (no kernel ever waits on another kernel), then copies
+# the other ranks' slices out of their contexts.  Everything else is the product path: sph_set_partition, the
+# range-restricted partner search / pair sums / walk, the exchange points, the replicated update.
+# ------------------------------------------------------------------------------------------------
+class VirtualRanks:
+    def __init__(self, P, w, world, **kw):
+        import threading
+        import torch
+        self.torch, self.world = torch, world
+        self.bar = threading.Barrier(world)
+        self.slots = [None] * world
+        self.errors = []
+        self.ctx = []
+        for r in range(world):
+            cfg, mats = P.config_of(w, **kw)
+            c = P.sph_create(cfg, mats, stream=torch.cuda.Stream())
+            c.upload_workload(w)
+            c.set_partition(r, world, exchange=self._exchange(r))
+            self.ctx.append(c)
+
+    def _exchange(self, r):
+        torch = self.torch
+
+        def ex(tensors, slice_bytes):
+            torch.cuda.current_stream().synchronize()            # my slices are complete
+            self.slots[r] = tensors
+            self.bar.wait()
+            for q in range(self.world):
+                if q == r:
+                    continue
+                for mine, theirs, sb in zip(tensors, self.slots[q], slice_bytes):
+                    mine[q * sb:(q + 1) * sb].copy_(theirs[q * sb:(q + 1) * sb])
+            torch.cuda.current_stream().synchronize()
+            self.bar.wait()                                      # nobody overwrites a slice somebody still reads
+        return ex
+
+    def run(self, fn):
+        """fn(ctx) on every rank, one thread per rank; returns the list of results"""
+        import threading
+        out = [None] * self.world
+
+        def body(r):
+            try:
+                out[r] = fn(self.ctx[r])
+            except BaseException as e:                           # noqa: BLE001 - reported by the main thread
+                self.errors.append((r, e))
+                self.bar.abort()
+
+        ts = [threading.Thread(target=body, args=(r,)) for r in range(self.world)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join()
+        if self.errors:
+            raise self.errors[0][1]
+        return out
+
+    def close(self):
+        for c in self.ctx:
+            c.close()
+
+
+@pytest.mark.parametrize("name,world", [("C5-twin", 2), ("C5-twin", 3), ("C2-twin", 2), ("C1x-twin", 4), ("blob3d", 5), ("C6-twin", 2)])
+def test_sharded_evaluation_and_step_equal_single_gpu_bit_for_bit(P, name, world):
+    w = CASES[name]()
+    h_iters = 1 if name == "C2-twin" else 0                       # C2: eq. 73 + density sum -> replicated lists
+    single = make_ctx(P, w, h_iters=h_iters)
+    single.evaluate()
+    want_eval = single.download()
+    single.step(w.dt)
+    single.step(w.dt)
+    want_step = single.download()
+    single.close()
+
+    vr = VirtualRanks(P, w, world, h_iters=h_iters)
+
+    def job(ctx):
+        ctx.evaluate()
+        a = ctx.download()
+        nb = ctx.get_neighbours()
+        ctx.step(w.dt)
+        ctx.step(w.dt)
+        return a, ctx.download(), nb
+
+    res = vr.run(job)
+    off_all, idx_all = [], []
+    for r, (a, b, (off, idx)) in enumerate(res):
+        for k in want_eval:                                       # every rank ends with the complete arrays
+            assert np.array_equal(a[k], want_eval[k]), (r, "evaluate", k)
+        for k in want_step:
+            assert np.array_equal(b[k], want_step[k]), (r, "step", k)
+    # partner lists are rank-local: together the ranks' slices hold every particle's list exactly once (unless replicated)
+    if h_iters == 0:
+        counts = np.stack([np.diff(off) for _, _, (off, _) in res])
+        assert np.array_equal(counts.sum(axis=0), want_eval["nb_count"])
+        assert np.all((counts > 0).sum(axis=0) <= 1)
+    vr.close()

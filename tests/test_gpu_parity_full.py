@@ -102,6 +102,14 @@ def test_c5_full_size(P):
     assert np.all(np.abs(g["ag"]).sum(axis=0) > 0.0)
 
 
+def test_c6_full_size(P):
+    w = sph_inputs.make("C6", twin=True)                     # 400 116 particles: basalt core + ice mantle vs basalt body
+    g, off = _full_case(P, w, 25)
+    assert np.bincount(np.diff(off)).argmax() == 80
+    ice = w.mat == 1
+    assert ice.any() and (~ice).any() and np.abs(g["ddmg"][ice]).max() > 0 and np.abs(g["ddmg"][~ice]).max() > 0
+
+
 def test_c1_full_size(P):
     w = sph_inputs.make("C1", twin=True)                     # 4 398 particles: brute force is affordable
     ctx = make_ctx(P, w, h_iters=0)

@@ -285,3 +285,25 @@ def test_gravity_accuracy_reading_U32(scale, bound5):
     assert 1e-3 < med[0.5] <= bound5          # the north_star bound is out of reach for monopoles at 0.5 ...
     assert med[0.3] <= 1e-3                   # ... and met at 0.3
     assert med[0.5] / med[0.3] >= (0.5 / 0.3) ** 2 * 0.8 and med[0.3] / med[0.15] >= 4.0 * 0.8   # >= theta^2 scaling
+
+
+def test_two_material_workload_c6_follows_the_papers_setup():
+    """sph_inputs.c6_ice_mantle against PAPER.md:592-615 (section 5.1, Tables 1-2): one Ceres mass each, basalt core with a
+    30 wt-% ice mantle (R_T = 509 km) against solid basalt (R_P = 437 km); every brittle particle of either material
+    holds at least one flaw drawn from ITS material's Weibull set over ITS material's volume."""
+    w = si.make("C6", scale=0.05)
+    tgt = np.arange(w.n) < w.meta["n_target"]
+    assert abs(w.meta["r_target"] / 509e3 - 1) < 2e-3 and abs(w.meta["r_projectile"] / 437e3 - 1) < 2e-3     # as printed
+    m_t, m_p = w.m[tgt].sum(), w.m[~tgt].sum()
+    assert abs(m_t / 9.43e20 - 1) < 0.03 and abs(m_p / 9.43e20 - 1) < 0.03                                    # lattice sampling
+    ice = w.mat == 1
+    assert not ice[~tgt].any() and abs(w.m[ice].sum() / m_t - 0.30) < 0.02                                    # 30 wt-% mantle
+    assert np.all(w.rho[ice] == 917.0) and np.all(w.rho[~ice] == 2700.0)                                      # Table 1
+    cnt = np.diff(w.flaw_off)
+    assert cnt.min() >= 1
+    dx = w.meta["dx"]
+    for k, (k_w, m_w) in si.WEIBULL_T2.items():
+        sel = np.flatnonzero(w.mat == k)
+        eps = np.sort(np.concatenate([w.flaw_eps[w.flaw_off[a]:w.flaw_off[a + 1]] for a in sel]))
+        want = (np.arange(1, eps.size + 1) / (k_w * sel.size * dx ** 3)) ** (1.0 / m_w)                      # eq. 45 per material
+        assert np.array_equal(eps, want)
