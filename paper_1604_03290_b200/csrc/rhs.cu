@@ -182,7 +182,12 @@ __device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02
     }
 }
 
+#ifndef PR_WARPS
 #define PR_WARPS 1
+#endif
+#ifndef PR_MINBLOCKS
+#define PR_MINBLOCKS 1            // resident blocks per SM the register allocation must allow (1 = no cap)
+#endif
 #define PR_STRIDE 18            // doubles between staged records (144 B): 16-byte reads by lane are conflict-free
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {
@@ -199,7 +204,7 @@ __device__ __forceinline__ void cp_async_wait1() { asm volatile("cp.async.wait_g
 // reads ITS partner's record from shared memory (144-byte stride: conflict-free).
 // EXTRA: artificial stress (eqs. 35-38, reading U25) and/or the XSPH sum (eq. 40, reading U26).
 template <int D, bool SOLID, bool VARH, bool EXTRA>
-__global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(Dev d, const sph_material *mats) {
+__global__ void __launch_bounds__(PR_WARPS * 32, PR_MINBLOCKS) k_pairs(Dev d, const sph_material *mats) {
     constexpr int NS = (D == 3) ? 6 : 3;                 // independent stress components
     constexpr int SI[6] = {0, 1, (D == 3) ? 2 : 3, 3, 4, 5};   // 2-D: xx xy yy -> 0 1 3
     __shared__ __align__(16) double s_buf[PR_WARPS][2][32 * PR_STRIDE];
