@@ -281,11 +281,11 @@ __global__ void __launch_bounds__(PR_WARPS * 32, PR_MINBLOCKS) k_pairs(Dev d, co
                 r2 += dx[a] * dx[a];
                 vr += dvv[a] * dx[a];
             }
-            const double rinv = (r2 > 0.0) ? rsqrt(r2) : 0.0;
+            const double rinv = (r2 > 0.0) ? rsqrt_fast(r2) : 0.0;     // a coincident partner contributes nothing
             const double r = r2 * rinv;
             double iH = iHi, fac = fac_i;
             if (VARH) {
-                iH = 1.0 / (0.5 * (Hi + hb));
+                iH = div_fast(1.0, 0.5 * (Hi + hb));
                 fac = 6.0 * KNorm<D>::s * ((D == 3) ? (iH * iH) * (iH * iH) : iH * iH * iH);
             }
             const double q = r * iH;
@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32, PR_MINBLOCKS) k_pairs(Dev d, co
             if (vr < 0.0) {                                   // eqs. 32-33, approaching pairs only
                 const double Hb = 0.5 * (Hi + hb), cb = 0.5 * (csi + csb), rb = 0.5 * (rhoi + rhob);
                 const double den = r2 + d.av_eps * Hb * Hb;
-                const double inv = 1.0 / (den * rb);
+                const double inv = div_fast(1.0, den * rb);
                 const double nu = Hb * vr * rb * inv;
                 Pi = nu * (d.av_beta * nu - d.av_alpha * cb) * den * inv;
             }
