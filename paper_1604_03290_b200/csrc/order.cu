@@ -225,6 +225,7 @@ __global__ void k_gather(Dev d) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     int o = d.perm[i];
+    d.iperm[o] = i;
     for (int a = 0; a < 3; ++a) {
         d.sx[a][i] = (a < d.D) ? d.x[a][o] : 0.0;
         d.sv[a][i] = (a < d.D) ? d.v[a][o] : 0.0;

@@ -100,6 +100,7 @@ struct Dev {
     int *idx[2];                // idx[cur][i] = original index of sorted i (perm)
     u64 *keys;                  // sorted keys (alias of key[cur] after the sort)
     int *perm;                  // alias of idx[cur]
+    int *iperm;                 // inverse: iperm[original] = sorted index (written by the reorder)
     unsigned *hist;             // radix histograms
     double *partial;            // bbox partials
     DevRoot *root;
