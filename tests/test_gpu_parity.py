@@ -755,3 +755,32 @@ def test_sharded_evaluation_and_step_equal_single_gpu_bit_for_bit(P, name, world
         assert np.array_equal(counts.sum(axis=0), want_eval["nb_count"])
         assert np.all((counts > 0).sum(axis=0) <= 1)
     vr.close()
+
+
+def test_nccl_all_gather_call_on_device_memory(P):
+    """The binding's all-gather on CUDA memory through torch.distributed's NCCL backend, with the one rank this box
+    has: checks the call itself (uint8 views over raw device pointers, in-place input/output aliasing, the library's
+    stream) that `Context.set_partition` uses for real multi-GPU runs.  The multi-rank data movement is covered on
+    CPU (tests/test_sharding_cpu.py) and with virtual ranks above."""
+    import subprocess
+    import sys
+    code = r'''
+import os, torch, torch.distributed as dist
+import paper_1604_03290_b200 as P
+from paper_1604_03290_b200.binding import device_bytes
+os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29531", RANK="0", WORLD_SIZE="1")
+dist.init_process_group("nccl", rank=0, world_size=1)
+st = torch.cuda.Stream()
+with torch.cuda.stream(st):
+    a = torch.arange(4096, dtype=torch.float64, device="cuda")
+    want = a.clone()
+    t = device_bytes(torch, a.data_ptr(), a.numel() * 8, torch.device("cuda", 0))
+    P.all_gather_slices([t], [a.numel() * 8], 0)
+st.synchronize()
+assert torch.equal(a, want)
+dist.destroy_process_group()
+print("nccl-ok")
+'''
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
+                         cwd=__import__("os").path.dirname(__import__("os").path.dirname(__import__("os").path.abspath(__file__))))
+    assert "nccl-ok" in out.stdout, out.stderr[-2000:]
