@@ -181,9 +181,17 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
         const int skip = sl.x, lo = sl.y;
         const bool act = (next == cur);
         const float reach = VH ? __fmul_ru(0.5f, __fadd_ru(Hf, r1.z)) * 1.000001f : Hf;
-        bool ov = act && (__fsub_rd(r0.x, xhi) <= reach) && (__fsub_rd(xlo, r0.w) <= reach) &&
-                  (__fsub_rd(r0.y, yhi) <= reach) && (__fsub_rd(ylo, r1.x) <= reach);
-        if (D == 3) ov = ov && (__fsub_rd(r0.z, zhi) <= reach) && (__fsub_rd(zlo, r1.y) <= reach);
+        // squared distance from the particle to the box, a LOWER bound (differences and products rounded down),
+        // against reach^2 rounded up: the ball around the particle, not the cube around it (the corners of the
+        // cube admit a quarter more boxes)
+        const float ex = fmaxf(fmaxf(__fsub_rd(r0.x, xhi), __fsub_rd(xlo, r0.w)), 0.0f);
+        const float ey = fmaxf(fmaxf(__fsub_rd(r0.y, yhi), __fsub_rd(ylo, r1.x)), 0.0f);
+        float d2 = __fmaf_rd(ey, ey, __fmul_rd(ex, ex));
+        if (D == 3) {
+            const float ez = fmaxf(fmaxf(__fsub_rd(r0.z, zhi), __fsub_rd(zlo, r1.y)), 0.0f);
+            d2 = __fmaf_rd(ez, ez, d2);
+        }
+        const bool ov = act && (d2 <= __fmul_ru(reach, reach));
         if (skip >= 0) {
             if (act) next = ov ? cur + 1 : skip;
         } else {
