@@ -8,8 +8,8 @@ list of PAPER.md:693) and two updates.  metric = particle-updates/s = N * RHS ev
 (SURVEY.md 8(d)).  Prints ONE JSON line (contract in DESIGN.md "Measurement").
 
   value         device-resident state, CUDA-event time of exactly K steps, max over ranks
-  e2e           the same step through the C ABI with HOST buffers: sph_upload (pinned host state) ->
-                sph_step -> sph_download (host state) inside the timed region
+  e2e           the same step through the C ABI with HOST buffers: sph_upload (pinned host state: x v rho u S dmg h
+                n_act) -> sph_step -> sph_download (host state) inside the timed region
   roofline      dominant kernel of the step, timed live by the library's CUDA-event stage brackets
   cpu_baseline  the CPU oracle (oracle/, tree mode, as it stands) on a bounded sample, rank 0, N=1: on all host
                 cores and (value_1core) on one core, the paper's own comparison
@@ -223,17 +223,16 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     host = dict(x=pin((3, n), torch.float64), v=pin((3, n), torch.float64), rho=pin((n,), torch.float64),
                 u=pin((n,), torch.float64), S=pin((6, n), torch.float64), dmg=pin((n,), torch.float64),
                 h=pin((n,), torch.float64), n_act=pin((n,), torch.int32))
-    const = dict(m=pin((n,), torch.float64), mat=pin((n,), torch.int32))
-    const["m"].numpy()[:] = w.m
-    const["mat"].numpy()[:] = w.mat
     ctx.download(tuple(host), out=host)                     # current state -> host (untimed)
-    h2d = sum(t.numel() * t.element_size() for t in list(host.values()) + list(const.values()))
+    # the step's input is the STATE (x v rho u S dmg h n_act); masses, material indices and the flaw table are
+    # parameters of the run, uploaded once with the workload (sph_upload leaves NULL members unchanged)
+    h2d = sum(t.numel() * t.element_size() for t in host.values())
     d2h = sum(t.numel() * t.element_size() for t in host.values())
     if w.dim == 2:
         h2d -= 2 * n * 8                                    # z rows of x and v are not copied in 2-D
 
     def e2e_step():
-        ctx.upload(device=False, **host, **const)
+        ctx.upload(device=False, **host)
         ctx.step(w.dt)
         ctx.download(tuple(host), out=host)                 # synchronises (host destination)
 
