@@ -85,7 +85,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.status = b.take<DevStatus>(1);
     for (int k = 0; k < 2; ++k) { z.nkey[k] = b.take<u64>(n); z.nhi[k] = b.take<int>(n); }
     z.nlevel = b.take<int>(n); z.nlo = b.take<int>(n); z.nhi_s = b.take<int>(n); z.nskip = b.take<int>(n);
-    z.nparent = b.take<int>(n); z.ncc = b.take<int>(n); z.nready = b.take<int>(n);
+    z.nparent = b.take<int>(n); z.ncc = b.take<int>(n); z.nready = b.take<int>(n); z.nord = b.take<int>(n);
     z.child = b.take<int>(n * NC);
     z.child_lo = b.take<int>(n * (NC + 1));
     z.nmass = b.take<double>(n);

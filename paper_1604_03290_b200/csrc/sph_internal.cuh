@@ -41,10 +41,10 @@ struct DevRoot {
     double pad[3];
 };
 
-// One record of the partner-search stream (neigh.cu): the octree cells that hold more than
-// SPH_BUCKET particles ("big" cells) and buckets of <= SPH_BUCKET Morton-consecutive particles, in
-// depth-first pre-order.  skip >= 0: big cell, index of the first record after its subtree;
-// skip < 0: bucket of -skip particles starting at sorted index lo.
+// One item of the search tree (neigh.cu): the octree cells that hold more than SPH_BUCKET particles
+// ("big" cells) and buckets of <= SPH_BUCKET Morton-consecutive particles; the child items of a cell are
+// contiguous, item 0 is the root.  skip >= 0: big cell, skip = index of its first child item, lo = number
+// of child items; skip < 0: bucket of -skip particles starting at sorted index lo.
 #define PR_REC 16
 #define SPH_BUCKET 16       // <= 32 (one lane stages one member); 16 measured best on C4/C5 (32: +11 %, 8: +14 %)
 struct __align__(16) SearchItem {
@@ -111,6 +111,7 @@ struct Dev {
     int *nlevel, *nlo, *nhi_s;  // per node
     int *nskip;                 // first node after the subtree (pre-order)
     int *nparent, *ncc, *nready; // parent cell (-1 root), number of child CELLS, children finished (k_moments)
+    int *nord;                  // search tree: ordinal of a big cell among its parent's items
     int *child;                 // NC per node: >=0 node, -1 empty, -2 leaf
     int *child_lo;              // NC+1 per node
     double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
@@ -120,7 +121,7 @@ struct Dev {
     GravMeta *gmeta;
     unsigned *gcnt, *gfirst;    // per cell: number of child records, index of the first
     double *gthr;               // 32 acceptance thresholds on r^2 (eq. 50), by record kind
-    u64 *bmark, *bscan;         // n+1 each: low word bucket starts, high word big cells per lo; scan
+    u64 *bmark, *bscan;         // n+1 each: bucket starts (parent | ordinal | length); child-item counts and their scan
     u64 *scan_tmp;              // scratch of the prefix sums
     // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
     int *nb;
