@@ -551,10 +551,10 @@ def main():
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures under profiles/ (filled in per round; None = not captured yet).
 TRAFFIC_NCU = {
-    # profiles/r1e_c5.md: k_gravity<3,4,2,0> 0.317 GB read + 0.084 GB written per launch
-    ("C5", "gravity"): 401.0e6,
-    ("C5", "pairs"): 3147.3e6,
-    ("C5", "neighbours"): 2919.0e6,
+    # profiles/r2_c5.md: k_gravity<3,4,2,0,0> 0.318 GB read + 0.084 GB written per launch
+    ("C5", "gravity"): 402.6e6,
+    ("C5", "pairs"): 3152.5e6,          # profiles/r2_c5.md
+    ("C5", "neighbours"): 2755.4e6,
 }
 
 if __name__ == "__main__":
