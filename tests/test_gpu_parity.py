@@ -325,6 +325,17 @@ def test_degenerate_inputs(P):
     assert ctx.get_tree()["level"].size == 0
     check_neighbours(ctx, o["nb_off"], o["nb_idx"])
     check_rates(w, g, o)
+    # a leaf of 101 coincident particles inside an ordinary cloud: the search tree cuts it into runs of 16 and the
+    # walk's multi-particle leaf sums them one by one
+    w = sph_inputs.random_blob(1500, dim=3, seed=15)
+    w.x[:, 700:800] = w.x[:, [42]]
+    ctx = make_ctx(P, w, max_neighbours=512)
+    ctx.evaluate()
+    g = ctx.download()
+    o = orc.evaluate(w, mode="brute")
+    check_order_and_tree(P, ctx, w)
+    check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    check_rates(w, g, o)
     w = base.copy()
     w.h[:] = 1e-6                                        # nobody has partners: every sum is empty
     ctx = make_ctx(P, w)
