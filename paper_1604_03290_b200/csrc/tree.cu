@@ -48,7 +48,7 @@ __global__ void k_find_nodes(Dev d) {
             if ((d.keys[lo] >> (shift - d.D)) == (ka >> (shift - d.D))) {
                 emit = true;
                 hi = (lvl == 0) ? d.n : lower_bound_key(d.keys, i + 1, d.n, cell0 + (1ull << shift));
-                nk = ((u64)lo << 8) | (u64)lvl;
+                nk = ((u64)lo << 5) | (u64)lvl;                             // level 0..21 in 5 bits
             }
         }
     }
@@ -71,12 +71,12 @@ __global__ void k_fill_nodes(Dev d, const u64 *__restrict__ nkey, const int *__r
     if (nd >= nn) return;
     const int D = d.D, NC = 1 << D;
     const u64 nk = nkey[nd];
-    const int lo = (int)(nk >> 8), lvl = (int)(nk & 255u), hi = nhi[nd];
+    const int lo = (int)(nk >> 5), lvl = (int)(nk & 31u), hi = nhi[nd];
     d.nlo[nd] = lo; d.nhi_s[nd] = hi; d.nlevel[nd] = lvl;
     const double s = ldexp(d.root->s0, -lvl);               // eq. 68 (exact)
     d.ns2[nd] = __dmul_rn(s, s);
     {   // skip index: first node whose range starts at or after hi (nodes are sorted by (lo, level))
-        const u64 want = (u64)hi << 8;
+        const u64 want = (u64)hi << 5;
         int l2 = nd + 1, h2 = nn;
         while (l2 < h2) { int mid = (l2 + h2) >> 1; if (nkey[mid] < want) l2 = mid + 1; else h2 = mid; }
         d.nskip[nd] = l2;
@@ -100,7 +100,7 @@ __global__ void k_fill_nodes(Dev d, const u64 *__restrict__ nkey, const int *__r
             u64 x = d.keys[b] ^ d.keys[e - 1];
             int common = D * d.L - (64 - __clzll((long long)x));
             int clvl = common / D;
-            u64 want = ((u64)b << 8) | (u64)clvl;
+            u64 want = ((u64)b << 5) | (u64)clvl;
             int l2 = nd + 1, h2 = nn;                       // children follow their parent in pre-order
             while (l2 < h2) { int mid = (l2 + h2) >> 1; if (nkey[mid] < want) l2 = mid + 1; else h2 = mid; }
             code = l2;
@@ -208,7 +208,7 @@ void sph_stage_tree(sph_ctx *ctx) {
     k_zero_status<<<1, 1, 0, ctx->stream>>>(d);
     k_find_nodes<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
     ctx->launches += 2;
-    int bits = 8, t = n;
+    int bits = 5, t = n;                     // key = first particle << 5 | level: one radix pass less for n < 2^19
     while (t > 0) { ++bits; t >>= 1; }
     int cur = 0;
     sph_radix_sort(ctx, d.nkey, d.nhi, n, &d.status->n_nodes, bits, &cur);
