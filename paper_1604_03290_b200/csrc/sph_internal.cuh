@@ -27,7 +27,7 @@ struct DevStatus {
     u64 n_inter;        // accepted pseudo-particles + direct particles, per particle, summed (A11)
     u64 n_visit;        // nodes whose opening test a particle evaluated, summed               (A11)
     u64 n_open;         // of those, the cells the particle opened (did not accept), summed   (A11)
-    int n_items;        // records of the partner-search stream
+    int n_items;        // items of the search tree (neigh.cu)
     int pad;
     u64 rkerr;          // bit pattern of the error estimate of eq. 63 (sph_step_rk3)
     u64 dtlim[3];       // bit patterns of the three time-step limits (positive doubles order like integers)
@@ -115,7 +115,7 @@ struct Dev {
     int *child;                 // NC per node: >=0 node, -1 empty, -2 leaf
     int *child_lo;              // NC+1 per node
     double *nmass, *ncom[3], *nbmin[3], *nbmax[3], *nhmax, *ns2;
-    // ---- partner-search stream ----
+    // ---- search tree of the partner search ----
     SearchItem *items;          // up to 2n records
     GravRec *grec;              // n + n_nodes records
     GravMeta *gmeta;
