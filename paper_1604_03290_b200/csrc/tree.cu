@@ -14,6 +14,8 @@
 //                  only), tight bounding box and hmax.  Children are
 //                  summed in octant order, every operation rounded separately (reading U15), so
 //                  that the opening decisions of the gravity walk are reproducible bit for bit.
+#include <cuda/atomic>
+
 #include "sph_internal.cuh"
 
 __device__ __forceinline__ int lower_bound_key(const u64 *__restrict__ k, int lo, int hi, u64 v) {
@@ -173,10 +175,10 @@ __global__ void k_moments(Dev d, int hmax_only) {
         cell_moments(d, nd, hmax_only != 0);
         const int parent = d.nparent[nd];
         if (parent < 0) return;
-        __threadfence();
-        const int done = atomicAdd(&d.nready[parent], 1) + 1;
+        // release my cell, acquire the siblings' cells: one acq_rel read-modify-write at device scope
+        cuda::atomic_ref<int, cuda::thread_scope_device> ready(d.nready[parent]);
+        const int done = ready.fetch_add(1, cuda::std::memory_order_acq_rel) + 1;
         if (done != d.ncc[parent]) return;
-        __threadfence();
         nd = parent;
     }
 }
