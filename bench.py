@@ -8,8 +8,9 @@ list of PAPER.md:693) and two updates.  metric = particle-updates/s = N * RHS ev
 (SURVEY.md 8(d)).  Prints ONE JSON line (contract in DESIGN.md "Measurement").
 
   value         device-resident state, CUDA-event time of exactly K steps, max over ranks
-  e2e           the same step through the C ABI with HOST buffers: sph_upload (pinned host state: x v rho u S dmg h
-                n_act) -> sph_step -> sph_download (host state) inside the timed region
+  e2e           the same step through the C ABI with HOST buffers: sph_step_host (= sph_upload of the pinned host state
+                x v rho u S dmg h n_act + sph_step, the copies on a second stream beside the first evaluation) ->
+                sph_download (host state) inside the timed region
   roofline      dominant kernel of the step, timed live by the library's CUDA-event stage brackets
   cpu_baseline  the CPU oracle (oracle/, tree mode, as it stands) on a bounded sample, rank 0, N=1: on all host
                 cores and (value_1core) on one core, the paper's own comparison
@@ -232,8 +233,7 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
         h2d -= 2 * n * 8                                    # z rows of x and v are not copied in 2-D
 
     def e2e_step():
-        ctx.upload(device=False, **host)
-        ctx.step(w.dt)
+        ctx.step_host(w.dt, **host)                         # sph_step_host: upload + step, the copies beside the first evaluation
         ctx.download(tuple(host), out=host)                 # synchronises (host destination)
 
     e2e_step()                                              # warm-up

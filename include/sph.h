@@ -165,6 +165,18 @@ int sph_evaluate(sph_ctx *ctx);
  * sph_create, the kernels are launched one by one. */
 int sph_step(sph_ctx *ctx, double dt);
 
+/* sph_upload(ctx, src, 0) followed by sph_step(ctx, dt) as ONE call, for a caller that feeds every step from HOST
+ * memory: the same state afterwards, bit for bit.  A second stream copies src while the first stream works: positions,
+ * h and masses go first, the order, the tree, the partner search and the walk (eqs. 50-51) -- which
+ * read nothing else -- run beside the copy of the other members, then those are gathered, the base copy of eq. 52 is
+ * taken and the SPH sums follow (the stages of the first evaluation are independent of one another apart from that
+ * order).  src: HOST pointers as for sph_upload (NULL members keep their device values); page-locked buffers are needed
+ * for the copies to overlap.  The call returns when everything is enqueued: src must stay unchanged until a call
+ * that synchronises (sph_sync, sph_download to host buffers).  The same src pointers and dt twice in a row: the whole
+ * sequence, copies included, is captured into a CUDA graph and replayed on later calls.  With stage timing, decoupled
+ * gravity or a partition set it is exactly sph_upload + sph_step. */
+int sph_step_host(sph_ctx *ctx, const sph_state_in *src, double dt);
+
 /* One step of the embedded Runge-Kutta scheme (eqs. 58-65): three complete
  * evaluations k1 = f(q), k2 = f(q + dt/2 k1), k3 = f(q - dt k1 + 2 dt k2); third-order result
  * q + dt (k1 + 4 k2 + k3)/6 (eq. 58), midpoint result q + dt k2 (eq. 62), error estimate

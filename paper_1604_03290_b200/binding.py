@@ -21,7 +21,7 @@ SPH_F_SOLID, SPH_F_PLASTIC, SPH_F_DAMAGE, SPH_F_GRAVITY, SPH_F_VARIABLE_H, SPH_F
 SPH_F_ART_STRESS, SPH_F_XSPH, SPH_F_RK3, SPH_F_EXPORT_GRADV = 64, 128, 256, 512
 
 EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sph_build_tree",
-           "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_download",
+           "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_step_host", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
            "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_partition", "sph_set_partition", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
@@ -91,6 +91,7 @@ def load_library():
     for name in ("sph_build_tree", "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_sync"):
         getattr(L, name).argtypes = [_vp]
     L.sph_step.argtypes = [_vp, C.c_double]
+    L.sph_step_host.argtypes = [_vp, C.POINTER(StateIn), C.c_double]
     L.sph_download.argtypes = [_vp, C.POINTER(StateOut), C.c_int]
     L.sph_get_order.argtypes = [_vp, _vp, _vp, _vp]
     L.sph_get_tree_size.argtypes = [_vp, C.POINTER(C.c_int32)]
@@ -198,10 +199,9 @@ class Context:
         self._keep.append(arr)
         return arr.ctypes.data
 
-    def upload(self, x=None, v=None, m=None, rho=None, u=None, S=None, dmg=None, h=None, mat=None, n_act=None,
-               flaw_off=None, flaw_eps=None, device=False):
-        """sph_upload.  Arrays: x, v (3, n); S (6, n); others (n,); numpy/host-tensor (device=False) or CUDA
-        torch tensors (device=True).  Pinned host tensors may be passed as numpy views."""
+    def _state_in(self, x=None, v=None, m=None, rho=None, u=None, S=None, dmg=None, h=None, mat=None, n_act=None,
+                  flaw_off=None, flaw_eps=None, device=False):
+        """sph_state_in of the given arrays (the arrays are kept alive in self._keep)."""
         t = self.torch
         f64, i32, i64 = (np.float64, t.float64), (np.int32, t.int32), (np.int64, t.int64)
         self._keep = []
@@ -222,9 +222,21 @@ class Context:
         s.flaw_off = self._in_ptr(flaw_off, i64, device)
         if flaw_eps is not None and int(self.cfg.n_flaws) > 0:
             s.flaw_eps = self._in_ptr(flaw_eps, f64, device)
+        return s
+
+    def upload(self, device=False, **arrays):
+        """sph_upload.  Arrays: x, v (3, n); S (6, n); others (n,); numpy/host-tensor (device=False) or CUDA
+        torch tensors (device=True).  Pinned host tensors may be passed as numpy views."""
+        s = self._state_in(device=device, **arrays)
         self._check(load_library().sph_upload(self.handle, C.byref(s), int(device)))
         if not device:
             self._keep = []
+
+    def step_host(self, dt, **arrays):
+        """sph_step_host: upload of HOST arrays (as for upload) and one step, the copies beside the first evaluation.
+        The arrays are referenced until the next call that synchronises: do not change them before that."""
+        s = self._state_in(device=False, **arrays)
+        self._check(load_library().sph_step_host(self.handle, C.byref(s), float(dt)))
 
     def upload_workload(self, w):
         self.upload(x=w.x, v=w.v, m=w.m, rho=w.rho, u=w.u, S=w.S, dmg=w.dmg, h=w.h, mat=w.mat, n_act=w.n_act,
@@ -436,6 +448,10 @@ def sph_evaluate(ctx):
 
 def sph_step(ctx, dt):
     ctx.step(dt)
+
+
+def sph_step_host(ctx, dt, **arrays):
+    ctx.step_host(dt, **arrays)
 
 
 def sph_download(ctx, fields=STATE_FIELDS + RATE_FIELDS, device=False, out=None):

@@ -453,6 +453,14 @@ size_t sph_workspace_bytes(const sph_config *cfg) {
     return carve(cfg, nullptr, nullptr, nullptr);
 }
 
+// the captured steps no longer describe what a step launches
+static void drop_graphs(sph_ctx *ctx) {
+    if (ctx->step_graph) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }
+    if (ctx->hstep_graph) { cudaGraphExecDestroy(ctx->hstep_graph); ctx->hstep_graph = nullptr; }
+    ctx->last_dt = ctx->graph_dt = -1.0;
+    ctx->hlast_dt = ctx->hgraph_dt = -1.0;
+}
+
 int sph_create(const sph_config *cfg, const sph_material *materials, void *d_workspace, size_t workspace_bytes,
                void *cuda_stream, sph_ctx **out) {
     if (!out) return SPH_ERR_ARG;
@@ -498,9 +506,15 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     sph_sort_init();
     c->step_graph = nullptr;
     c->last_dt = c->graph_dt = -1.0;
+    c->hstep_graph = nullptr;
+    c->hlast_dt = c->hgraph_dt = -1.0;
     c->graphs_off = (getenv("SPH_NO_GRAPH") != nullptr);
+    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&c->ev_geom, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&c->ev_rest, cudaEventDisableTiming);
     int rc = check_cuda(c, "sph_create");
-    if (rc != SPH_OK) { delete e; return rc; }
+    if (rc != SPH_OK) { sph_destroy(c); return rc; }
     *out = c;
     return SPH_OK;
 }
@@ -508,7 +522,11 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
 void sph_destroy(sph_ctx *ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
-    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_geom) cudaEventDestroy(ctx->ev_geom);
+    if (ctx->ev_rest) cudaEventDestroy(ctx->ev_rest);
+    drop_graphs(ctx);
     delete ctx->timing;
     delete ext(ctx);
 }
@@ -548,8 +566,7 @@ const char *sph_timing_name(int stage) {
 int sph_counters_enable(sph_ctx *ctx, int on) {
     if (!ctx) return SPH_ERR_ARG;
     ctx->count_work = on ? 1 : 0;
-    if (ctx->step_graph) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }   // another kernel variant
-    ctx->last_dt = ctx->graph_dt = -1.0;
+    drop_graphs(ctx);                        // another kernel variant
     return SPH_OK;
 }
 
@@ -654,8 +671,7 @@ int sph_set_partition(sph_ctx *ctx, int rank, int world, sph_exchange_fn fn, voi
     ctx->xfn = (world > 1) ? fn : nullptr; ctx->xuser = user;
     ctx->d.r_lo = (int)lo; ctx->d.r_hi = (int)hi;
     ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
-    if (ctx->step_graph) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }
-    ctx->last_dt = ctx->graph_dt = -1.0;
+    drop_graphs(ctx);
     return SPH_OK;
 }
 
@@ -839,6 +855,108 @@ int sph_step(sph_ctx *ctx, double dt) {
     ctx->graph_dt = dt;
     ctx->graph_launches = ctx->launches - l0;
     if (cudaGraphLaunch(exec, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
+    return SPH_OK;
+}
+
+// ---- sph_step_host: upload and step as one call, the copies beside the first evaluation ----
+// part 0: what the tree, the partner search and the walk read; part 1: the rest of sph_upload's members
+static void upload_part(sph_ctx *ctx, const sph_state_in *s, cudaStream_t st, int part) {
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    auto cp = [&](void *dst, const void *src, size_t bytes) {
+        if (src && bytes) cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    if (part == 0) {
+        for (int a = 0; a < d.D; ++a) cp(d.x[a], s->x[a], n * 8);
+        cp(d.h, s->h, n * 8); cp(d.m, s->m, n * 8);
+        cudaMemsetAsync(&d.status->err_nb_overflow, 0, 3 * sizeof(int), st);   // as sph_upload
+    } else {
+        for (int a = 0; a < d.D; ++a) cp(d.v[a], s->v[a], n * 8);
+        cp(d.rho, s->rho, n * 8); cp(d.u, s->u, n * 8); cp(d.dmg, s->dmg, n * 8);
+        for (int k = 0; k < 6; ++k) cp(d.S[k], s->S[k], n * 8);
+        cp(d.mat, s->mat, n * 4); cp(d.n_act, s->n_act, n * 4);
+        cp(d.flaw_off, s->flaw_off, (n + 1) * 8);
+        cp(d.flaw_eps, s->flaw_eps, (size_t)ctx->cfg.n_flaws * 8);
+    }
+}
+
+// The launches of sph_upload + sph_step with the first evaluation reordered: positions, h and masses arrive first and the
+// order, the tree, the partner search and the walk (which read nothing else) run while the second stream copies the rest;
+// then the remaining arrays are gathered, the base copy of eq. 52 is taken and the SPH sums follow.
+static int host_step_enqueue(sph_ctx *ctx, const sph_state_in *s, double dt) {
+    Dev &d = ctx->d;
+    const size_t n = (size_t)d.n;
+    int rc;
+    cudaEventRecord(ctx->ev_fork, ctx->stream);                   // the copies overwrite what earlier launches may still read
+    cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_fork, 0);
+    upload_part(ctx, s, ctx->copy_stream, 0);
+    cudaEventRecord(ctx->ev_geom, ctx->copy_stream);
+    upload_part(ctx, s, ctx->copy_stream, 1);
+    cudaEventRecord(ctx->ev_rest, ctx->copy_stream);
+    cudaStreamWaitEvent(ctx->stream, ctx->ev_geom, 0);
+    ctx->have_state = 1; ctx->have_tree = ctx->have_lists = ctx->have_rates = 0;
+    ctx->step_no = 1; ctx->grav_reuse = 0;
+    ctx->split_gather = 1;
+    sph_stage_order(ctx);
+    ctx->split_gather = 0;
+    sph_stage_tree(ctx);
+    ctx->have_tree = 1;
+    sph_stage_neigh(ctx);
+    ctx->have_lists = 1;
+    sph_stage_gravity(ctx);
+    ctx->have_rates |= 2;
+    cudaStreamWaitEvent(ctx->stream, ctx->ev_rest, 0);
+    sph_stage_gather_rest(ctx);
+    cudaMemcpyAsync(d.q0, d.x[0], 15 * n * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream);
+    sph_stage_rhs(ctx);
+    ctx->have_rates |= 1;
+    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), 0.5 * dt, 0);   // eq. 52
+    ctx->launches += 1;
+    if ((rc = sph_evaluate(ctx)) != SPH_OK) return rc;
+    k_update<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d, sph_dev_mats(ctx), dt, 1);         // eq. 53
+    ctx->launches += 1;
+    ctx->have_tree = ctx->have_lists = 0;
+    return check_cuda(ctx, "sph_step_host");
+}
+
+int sph_step_host(sph_ctx *ctx, const sph_state_in *s, double dt) {
+    if (!ctx || !s) return SPH_ERR_ARG;
+    // stage timing, decoupled gravity and sharded runs take the plain sequence
+    if (ctx->timing || ctx->cfg.gravity_every > 1 || ctx->world > 1 || !ctx->copy_stream) {
+        const int rc = sph_upload(ctx, s, 0);
+        return rc != SPH_OK ? rc : sph_step(ctx, dt);
+    }
+    const bool same = memcmp(&ctx->hlast_src, s, sizeof(*s)) == 0 && ctx->hlast_dt == dt;
+    if (ctx->hstep_graph && ctx->hgraph_dt == dt && memcmp(&ctx->hgraph_src, s, sizeof(*s)) == 0) {
+        if (cudaGraphLaunch(ctx->hstep_graph, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step_host (graph)");
+        ctx->launches += ctx->hgraph_launches;
+        ctx->have_state = 1; ctx->have_tree = ctx->have_lists = 0; ctx->have_rates = 3; ctx->step_no = 1;
+        return SPH_OK;
+    }
+    ctx->hlast_src = *s; ctx->hlast_dt = dt;
+    // the same buffers and dt twice in a row: capture the sequence (both streams) and replay it from then on
+    if (!same || ctx->graphs_off || cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+        cudaGetLastError();
+        return host_step_enqueue(ctx, s, dt);
+    }
+    const i64 l0 = ctx->launches;
+    const int rc = host_step_enqueue(ctx, s, dt);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(ctx->stream, &graph);
+    cudaGraphExec_t exec = nullptr;
+    if (rc != SPH_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (graph) cudaGraphDestroy(graph);
+        ctx->launches = l0;
+        ctx->graphs_off = 1;                     // nothing has run: do the step with plain launches
+        return host_step_enqueue(ctx, s, dt);
+    }
+    cudaGraphDestroy(graph);
+    if (ctx->hstep_graph) cudaGraphExecDestroy(ctx->hstep_graph);
+    ctx->hstep_graph = exec;
+    ctx->hgraph_dt = dt; ctx->hgraph_src = *s;
+    ctx->hgraph_launches = ctx->launches - l0;
+    if (cudaGraphLaunch(exec, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step_host (graph)");
     return SPH_OK;
 }
 

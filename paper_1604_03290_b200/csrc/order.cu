@@ -221,23 +221,35 @@ void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const in
 // ------------------------------------------------------------------------------------------
 // SoA gather into sorted order
 // ------------------------------------------------------------------------------------------
-__global__ void k_gather(Dev d) {
+// Two kernels: what the tree, the partner search and the walk read (positions, masses, h), and the rest of the
+// state.  sph_step_host (api.cu) runs the second one only when the later part of its upload has arrived.
+__global__ void k_gather_geom(Dev d) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     int o = d.perm[i];
     d.iperm[o] = i;
-    for (int a = 0; a < 3; ++a) {
-        d.sx[a][i] = (a < d.D) ? d.x[a][o] : 0.0;
-        d.sv[a][i] = (a < d.D) ? d.v[a][o] : 0.0;
-    }
+    for (int a = 0; a < 3; ++a) d.sx[a][i] = (a < d.D) ? d.x[a][o] : 0.0;
     d.sm[i] = d.m[o];
+    d.sh[i] = d.h[o];
+}
+
+__global__ void k_gather_rest(Dev d) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    int o = d.perm[i];
+    for (int a = 0; a < 3; ++a) d.sv[a][i] = (a < d.D) ? d.v[a][o] : 0.0;
     d.srho[i] = d.rho[o];
     d.su[i] = d.u[o];
-    d.sh[i] = d.h[o];
     d.smat[i] = d.mat[o];
     if (d.flags & SPH_F_SOLID)
         for (int k = 0; k < 6; ++k) d.sS[k][i] = d.S[k][o];
     if (d.flags & SPH_F_DAMAGE) d.sdmg[i] = d.dmg[o];
+}
+
+void sph_stage_gather_rest(sph_ctx *ctx) {
+    StageTimer tm(ctx, SPH_T_REORDER);
+    k_gather_rest<<<sph_ceil_div(ctx->d.n, 256), 256, 0, ctx->stream>>>(ctx->d);
+    ctx->launches += 1;
 }
 
 void sph_stage_order(sph_ctx *ctx) {
@@ -259,7 +271,10 @@ void sph_stage_order(sph_ctx *ctx) {
     d.keys = d.key[cur];
     d.perm = d.idx[cur];
     ctx->sort_cur = cur;
-    StageTimer tm(ctx, SPH_T_REORDER);
-    k_gather<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
-    ctx->launches += 1;
+    {
+        StageTimer tm(ctx, SPH_T_REORDER);
+        k_gather_geom<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
+        ctx->launches += 1;
+    }
+    if (!ctx->split_gather) sph_stage_gather_rest(ctx);
 }

@@ -168,6 +168,14 @@ struct sph_ctx {
     int graphs_off;
     i64 step_no;                // sph_step calls since the last upload (gravity_every)
     int grav_reuse;             // set by sph_step: sph_evaluate takes the stored accelerations
+    // sph_step_host: the upload runs on a second stream beside the geometric stages of the first evaluation
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_fork, ev_geom, ev_rest;
+    int split_gather;           // sph_stage_order gathers positions, masses and h only (sph_stage_gather_rest follows later)
+    cudaGraphExec_t hstep_graph;
+    double hgraph_dt, hlast_dt;
+    i64 hgraph_launches;
+    sph_state_in hgraph_src, hlast_src;
     char err[512];
 };
 
@@ -196,6 +204,7 @@ size_t sph_scan_scratch_elems(i64 n);
 
 // ---- per-stage entry points (each enqueues kernels on ctx->stream) ----
 void sph_stage_order(sph_ctx *ctx);     // A1 + A2
+void sph_stage_gather_rest(sph_ctx *ctx);   // second half of A2 when ctx->split_gather was set for sph_stage_order
 void sph_stage_tree(sph_ctx *ctx);      // A3 + A4
 void sph_stage_neigh(sph_ctx *ctx);     // A5
 void sph_stage_rhs(sph_ctx *ctx);       // A6-A10

@@ -462,6 +462,44 @@ def test_step_graph_replay_is_bit_identical(P, monkeypatch):
         assert np.array_equal(a[k], b[k]), k
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", ["C5-twin", "C2-twin", "C1-twin"])
+def test_step_host_equals_upload_then_step(P, case):
+    """sph_step_host = sph_upload + sph_step with the copies on a second stream beside the geometric stages of the
+    first evaluation (include/sph.h): the same state and rates bit for bit, from pinned host buffers, with plain
+    launches (first two calls), the captured graph (later calls) and after a change of dt."""
+    import torch
+    w = CASES[case]()
+    stream = torch.cuda.Stream()
+    cfg, mats = P.config_of(w)
+
+    def pinned(g):
+        out = {}
+        for k in P.STATE_FIELDS:
+            t = torch.from_numpy(np.ascontiguousarray(g[k])).pin_memory()
+            out[k] = t
+        return out
+
+    ref = P.sph_create(cfg, mats, stream=stream)
+    ref.upload_workload(w)
+    ctx = P.sph_create(cfg, mats, stream=stream)
+    ctx.upload_workload(w)                                   # masses, materials, flaws: parameters of the run
+    host = pinned(ref.download(P.STATE_FIELDS))
+    for k, dt in enumerate([w.dt, w.dt, w.dt, w.dt, 0.5 * w.dt, 0.5 * w.dt, 0.5 * w.dt]):
+        ref.upload(**{f: host[f] for f in host})
+        ref.step(dt)
+        a = ref.download()
+        ctx.step_host(dt, **host)
+        b = ctx.download()                                   # synchronises: the host buffers are free again
+        for f in a:
+            assert np.array_equal(a[f], b[f]), (k, f)
+        for f in host:                                       # next step from the new state, same buffers (graph replay)
+            host[f].copy_(torch.from_numpy(np.ascontiguousarray(a[f])))
+    assert ref.launch_count() == ctx.launch_count()
+    ref.close()
+    ctx.close()
+
+
 @pytest.mark.parametrize("name", ["C1x-twin", "C4-twin", "C2-twin"])
 def test_step_rk3_parity(P, name):
     """sph_step_rk3 (eqs. 58-65) against the oracle: error estimate, new step size, accepted state;
