@@ -98,6 +98,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.gcnt = b.take<unsigned>((c->flags & SPH_F_GRAVITY) ? n + 1 : 1);
     z.gfirst = b.take<unsigned>((c->flags & SPH_F_GRAVITY) ? n + 1 : 1);
     z.gthr = b.take<double>(32);
+    z.bbox_done = b.take<unsigned>(1);
     z.bmark = b.take<u64>(n + 1); z.bscan = b.take<u64>(n + 1);
     z.scan_tmp = b.take<u64>(sph_scan_scratch_elems((i64)n + 1) + 2);
     z.nb = b.take<int>(groups * (size_t)cfg_cap(c) * 32);
@@ -493,6 +494,7 @@ int sph_create(const sph_config *cfg, const sph_material *materials, void *d_wor
     for (int k = 0; k < cfg->n_materials; ++k) c->mats.m[k] = materials[k];
     cudaMemcpyAsync(e->mats_dev, &c->mats, sizeof(Mats), cudaMemcpyHostToDevice, c->stream);
     cudaMemsetAsync(d.status, 0, sizeof(DevStatus), c->stream);
+    cudaMemsetAsync(d.bbox_done, 0, sizeof(unsigned), c->stream);
     // defaults for state members never uploaded
     const size_t n = (size_t)d.n;
     cudaMemsetAsync(d.x[0], 0, 15 * n * sizeof(double), c->stream);

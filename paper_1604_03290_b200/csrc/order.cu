@@ -12,54 +12,85 @@
 #define SORT_WARPS (SORT_THREADS / 32)
 
 // ------------------------------------------------------------------------------------------
-// bounding box: per-block partial min/max, then one block finishes and derives s0 and scale
+// bounding box: per-block partial min/max; the last block to finish reduces them and derives s0 and scale
 // ------------------------------------------------------------------------------------------
-__global__ void k_bbox_partial(Dev d, int nblocks) {
-    __shared__ double smin[3][8], smax[3][8];
-    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n; i += gridDim.x * blockDim.x)
-        for (int a = 0; a < d.D; ++a) {
-            double v = d.x[a][i];
-            lo[a] = fmin(lo[a], v); hi[a] = fmax(hi[a], v);
-        }
-    for (int a = 0; a < 3; ++a)
-        for (int o = 16; o > 0; o >>= 1) {
-            lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
-            hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
-        }
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    if (l == 0) for (int a = 0; a < 3; ++a) { smin[a][w] = lo[a]; smax[a][w] = hi[a]; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int a = 0; a < 3; ++a) {
-            double mn = smin[a][0], mx = smax[a][0];
-            for (int k = 1; k < (int)(blockDim.x >> 5); ++k) { mn = fmin(mn, smin[a][k]); mx = fmax(mx, smax[a][k]); }
-            d.partial[(blockIdx.x * 3 + a) * 2 + 0] = mn;
-            d.partial[(blockIdx.x * 3 + a) * 2 + 1] = mx;
-        }
-    }
+// min / max as integers: the bit pattern of a double with the sign bit flipped (positive) or all bits flipped (negative)
+// orders like the value, and integer min / max cost one instruction where fmin / fmax of doubles cost four
+__device__ __forceinline__ u64 dbl_key(double v) {
+    const u64 b = (u64)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double key_dbl(u64 k) {
+    return __longlong_as_double((long long)((k >> 63) ? (k & 0x7fffffffffffffffull) : ~k));
 }
 
-__global__ void k_bbox_final(Dev d, int nblocks) {
-    // one warp
-    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-    for (int b = threadIdx.x; b < nblocks; b += 32)
-        for (int a = 0; a < 3; ++a) {
-            lo[a] = fmin(lo[a], d.partial[(b * 3 + a) * 2 + 0]);
-            hi[a] = fmax(hi[a], d.partial[(b * 3 + a) * 2 + 1]);
+// The last block to finish (counter in d.partial's tail) reduces the per-block partials and derives s0 and scale.
+__global__ void __launch_bounds__(256) k_bbox(Dev d, int nblocks, unsigned *done) {
+    __shared__ u64 smin[3][8], smax[3][8];
+    __shared__ bool last;
+    u64 lo[3] = {~0ull, ~0ull, ~0ull}, hi[3] = {0ull, 0ull, 0ull};
+    const int stride = gridDim.x * blockDim.x;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < d.n; i += 4 * stride) {           // four loads per axis in flight
+        for (int a = 0; a < d.D; ++a) {
+            const u64 k0 = dbl_key(d.x[a][i]), k1 = dbl_key(d.x[a][i + stride]), k2 = dbl_key(d.x[a][i + 2 * stride]),
+                      k3 = dbl_key(d.x[a][i + 3 * stride]);
+            lo[a] = min(min(lo[a], k0), min(k1, min(k2, k3)));
+            hi[a] = max(max(hi[a], k0), max(k1, max(k2, k3)));
         }
-    for (int a = 0; a < 3; ++a)
+    }
+    for (; i < d.n; i += stride)
+        for (int a = 0; a < d.D; ++a) { const u64 k = dbl_key(d.x[a][i]); lo[a] = min(lo[a], k); hi[a] = max(hi[a], k); }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    for (int a = 0; a < 3; ++a) {
         for (int o = 16; o > 0; o >>= 1) {
-            lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
-            hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+            lo[a] = min(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = max(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
         }
+        if (l == 0) { smin[a][w] = lo[a]; smax[a][w] = hi[a]; }
+    }
+    __syncthreads();
+    u64 *part = reinterpret_cast<u64 *>(d.partial);
+    if (threadIdx.x < 6) {
+        const int a = threadIdx.x >> 1, isx = threadIdx.x & 1;
+        u64 v = isx ? smax[a][0] : smin[a][0];
+        for (int k = 1; k < 8; ++k) v = isx ? max(v, smax[a][k]) : min(v, smin[a][k]);
+        part[(blockIdx.x * 3 + a) * 2 + isx] = v;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) last = (atomicAdd(done, 1u) == (unsigned)(nblocks - 1));
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (int a = 0; a < 3; ++a) { lo[a] = ~0ull; hi[a] = 0ull; }
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x)
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = min(lo[a], __ldcg(&part[(b * 3 + a) * 2 + 0]));
+            hi[a] = max(hi[a], __ldcg(&part[(b * 3 + a) * 2 + 1]));
+        }
+    for (int a = 0; a < 3; ++a) {
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = min(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = max(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+        if (l == 0) { smin[a][w] = lo[a]; smax[a][w] = hi[a]; }
+    }
+    __syncthreads();
     if (threadIdx.x == 0) {
+        double mn[3], mx[3];
+        for (int a = 0; a < 3; ++a) {
+            u64 l2 = smin[a][0], h2 = smax[a][0];
+            for (int k = 1; k < 8; ++k) { l2 = min(l2, smin[a][k]); h2 = max(h2, smax[a][k]); }
+            mn[a] = key_dbl(l2); mx[a] = key_dbl(h2);
+        }
         double s0 = 0.0;
-        for (int a = 0; a < d.D; ++a) s0 = fmax(s0, __dsub_rn(hi[a], lo[a]));   // eq. 67
+        for (int a = 0; a < d.D; ++a) s0 = fmax(s0, __dsub_rn(mx[a], mn[a]));   // eq. 67
         if (!(s0 > 0.0)) s0 = 1.0;
-        for (int a = 0; a < 3; ++a) d.root->xmin[a] = (a < d.D) ? lo[a] : 0.0;
+        for (int a = 0; a < 3; ++a) d.root->xmin[a] = (a < d.D) ? mn[a] : 0.0;
         d.root->s0 = s0;
         d.root->scale = __ddiv_rn(ldexp(1.0, d.L), s0);
+        *done = 0u;                                             // for the next launch
     }
 }
 
@@ -258,10 +289,9 @@ void sph_stage_order(sph_ctx *ctx) {
     int nb = min(sph_ceil_div(n, 256), 1024);
     {
         StageTimer tm(ctx, SPH_T_KEYS);
-        k_bbox_partial<<<nb, 256, 0, ctx->stream>>>(d, nb);
-        k_bbox_final<<<1, 32, 0, ctx->stream>>>(d, nb);
+        k_bbox<<<nb, 256, 0, ctx->stream>>>(d, nb, d.bbox_done);
         k_keys<<<sph_ceil_div(n, 256), 256, 0, ctx->stream>>>(d);
-        ctx->launches += 3;
+        ctx->launches += 2;
     }
     int cur = 0;
     {

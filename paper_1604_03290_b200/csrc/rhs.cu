@@ -50,41 +50,56 @@ __device__ __forceinline__ double yield_factor(const sph_material &mt, int flags
     return (3.0 * J2 > Y2) ? Y2 / (3.0 * J2) : 1.0;
 }
 
+#define PP_WARPS 8
 template <int D>
-__global__ void k_prepass(Dev d, const sph_material *mats) {
+__global__ void __launch_bounds__(PP_WARPS * 32) k_prepass(Dev d, const sph_material *mats) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.n) return;
-    const sph_material mt = mats[d.smat[i]];
-    const double rho = d.srho[i], u = d.su[i];
+    const int n = d.n;
+    const int ii = min(i, n - 1);                              // (a tail lane repeats the last particle and stores nothing)
+    const sph_material mt = mats[d.smat[ii]];
+    const double rho = d.srho[ii], u = d.su[ii];
     double p, cs;
     eos_eval(mt, rho, u, p, cs);
     double S[6] = {0, 0, 0, 0, 0, 0};
     if (d.flags & SPH_F_SOLID) {
-        for (int k = 0; k < 6; ++k) S[k] = d.sS[k][i];
+        for (int k = 0; k < 6; ++k) S[k] = d.sS[k][ii];
         if (D == 2) { S[2] = 0.0; S[4] = 0.0; S[5] = 0.0; }
         const double fY = yield_factor<D>(mt, d.flags, S);
         for (int k = 0; k < 6; ++k) S[k] *= fY;
     }
     double dd = 0.0;
-    if ((d.flags & SPH_F_DAMAGE) && mt.brittle) { const double g = d.sdmg[i]; dd = g * g * g; }
+    if ((d.flags & SPH_F_DAMAGE) && mt.brittle) { const double g = d.sdmg[ii]; dd = g * g * g; }
     const double phat = (p >= 0.0) ? p : (1.0 - dd) * p;
     const double ir2 = 1.0 / (rho * rho);
     double sg[6];
     for (int k = 0; k < 6; ++k) sg[k] = (1.0 - dd) * S[k];
     sg[0] -= phat; sg[3] -= phat;
     if (D == 3) sg[5] -= phat;
-    d.p[i] = p;
-    d.cs[i] = cs;
-    // packed 128-byte record read by the pair kernel (one cache line per partner)
-    double2 *rec = reinterpret_cast<double2 *>(d.prec + (size_t)i * PR_REC);
-    rec[0] = make_double2(d.sx[0][i], d.sx[1][i]);
-    rec[1] = make_double2((D == 3) ? d.sx[2][i] : 0.0, d.sv[0][i]);
-    rec[2] = make_double2(d.sv[1][i], (D == 3) ? d.sv[2][i] : 0.0);
-    rec[3] = make_double2(rho, d.sm[i] / rho);
-    rec[4] = make_double2(cs, d.sh[i]);
-    rec[5] = make_double2(sg[0] * ir2, sg[1] * ir2);
-    rec[6] = make_double2(sg[2] * ir2, sg[3] * ir2);
-    rec[7] = make_double2(sg[4] * ir2, sg[5] * ir2);
+    if (i < n) { d.p[i] = p; d.cs[i] = cs; }
+    // packed 128-byte record read by the pair kernel (one cache line per partner).  The 32 records of a warp go through
+    // shared memory (144-byte stride: conflict-free 16-byte accesses) and leave as 8 fully coalesced 512-byte stores;
+    // one lane storing its own record 16 bytes at a time touched 32 lines per store instruction.
+    __shared__ __align__(16) double s_rec[PP_WARPS][32 * 18];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (i < n) {
+        double2 *rec = reinterpret_cast<double2 *>(&s_rec[w][lane * 18]);
+        rec[0] = make_double2(d.sx[0][i], d.sx[1][i]);
+        rec[1] = make_double2((D == 3) ? d.sx[2][i] : 0.0, d.sv[0][i]);
+        rec[2] = make_double2(d.sv[1][i], (D == 3) ? d.sv[2][i] : 0.0);
+        rec[3] = make_double2(rho, d.sm[i] / rho);
+        rec[4] = make_double2(cs, d.sh[i]);
+        rec[5] = make_double2(sg[0] * ir2, sg[1] * ir2);
+        rec[6] = make_double2(sg[2] * ir2, sg[3] * ir2);
+        rec[7] = make_double2(sg[4] * ir2, sg[5] * ir2);
+    }
+    __syncwarp();
+    const int i0 = i - lane;                                   // first particle of the warp
+    double2 *out = reinterpret_cast<double2 *>(d.prec + (size_t)i0 * PR_REC);
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {
+        const int q = t * 32 + lane, r = q >> 3, sub = q & 7;  // record r of the warp, 16-byte part sub
+        if (i0 + r < n) out[q] = *reinterpret_cast<const double2 *>(&s_rec[w][r * 18 + sub * 2]);
+    }
 }
 
 template <int D> struct KNorm;

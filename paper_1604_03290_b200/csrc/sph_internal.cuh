@@ -121,6 +121,7 @@ struct Dev {
     GravMeta *gmeta;
     unsigned *gcnt, *gfirst;    // per cell: number of child records, index of the first
     double *gthr;               // 32 acceptance thresholds on r^2 (eq. 50), by record kind
+    unsigned *bbox_done;        // blocks of k_bbox that have finished (0 between launches)
     u64 *bmark, *bscan;         // n+1 each: bucket starts (parent | ordinal | length); child-item counts and their scan
     u64 *scan_tmp;              // scratch of the prefix sums
     // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
