@@ -79,7 +79,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.smat = b.take<int>(n);
     for (int k = 0; k < 2; ++k) { z.key[k] = b.take<u64>(n); z.idx[k] = b.take<int>(n); }
     z.iperm = b.take<int>(n);
-    z.hist = b.take<unsigned>(256 * ((n + 4095) / 4096) + 256);
+    z.hist = b.take<unsigned>(sph_sort_ws_words((i64)n));
     z.partial = b.take<double>(1024 * 6);
     z.root = b.take<DevRoot>(1);
     z.status = b.take<DevStatus>(1);

@@ -1,9 +1,12 @@
 // A1 + A2: root cube, Morton keys, LSD radix sort, SoA reorder.
 //   root cube:  PAPER.md:463-465 (eq. 67); min-corner anchored (reading U12)
 //   keys:       L bits per dimension, x lowest bit of each group (U13); ties by original index
-//   sort:       hand-written 8-bit LSD radix sort (histogram -> scan -> stable scatter)
+//   sort:       hand-written 8-bit LSD radix sort, one kernel per pass (digit counts of all passes up front, stable
+//               scatter with decoupled look-back over the tiles)
 //   reorder:    every state array gathered into Morton order so that the tree walks, the partner
 //               search and the pair sums read neighbouring particles from neighbouring addresses.
+#include <cuda/atomic>
+
 #include "sph_internal.cuh"
 
 #define SORT_THREADS 256
@@ -133,19 +136,57 @@ __global__ void k_keys(Dev d) {
 // ------------------------------------------------------------------------------------------
 // radix sort
 // ------------------------------------------------------------------------------------------
-__global__ void k_sort_hist(const u64 *__restrict__ kin, int n_host, const int *n_dev, int shift,
-                            unsigned *hist, int nblocks) {
-    __shared__ unsigned h[256];
+// One pass = ONE kernel ("onesweep": Adinets & Merrill 2022, restated).  The counts of every digit of every pass over
+// the whole input are taken once up front (k_sort_hist_all) and turned into the global start of every digit
+// (k_sort_bases).  In a pass a block takes the next tile (a ticket, so that tiles start in order), ranks its keys,
+// publishes the tile's digit counts and obtains the number of equal digits in all earlier tiles by looking back over the
+// published counts of its predecessors: a word holds a count and a state, AGGREGATE (this tile alone) or PREFIX (this tile
+// and everything before it); the walk back stops at the first PREFIX.  A tile waits only for tiles with smaller tickets,
+// which are resident or finished, so the chain always ends (tile 0 publishes a PREFIX at once).  Round 1's pass was a
+// histogram kernel, a three-kernel scan and the scatter: 40 launches for 8 passes, 11 now.
+#define SORT_MAX_PASSES 8
+#define SORT_LOOK 8                     // predecessors inspected per step of the look-back
+#define SORT_FLAG_A 0x40000000u
+#define SORT_FLAG_P 0x80000000u
+#define SORT_CNT_MASK 0x3fffffffu       // n <= 0x3fffffff (cfg_ok)
+
+// workspace (unsigned words): tickets [8, padded to 64] | digit counts / bases [8][256] | tile states [passes][tiles][256]
+__host__ __device__ inline size_t sort_ws_words(i64 n) { return 64 + SORT_MAX_PASSES * 256 + (size_t)SORT_MAX_PASSES * 256 * ((n + SORT_TILE - 1) / SORT_TILE); }
+size_t sph_sort_ws_words(i64 n) { return sort_ws_words(n); }
+
+__global__ void __launch_bounds__(256) k_sort_hist_all(const u64 *__restrict__ kin, int n_host, const int *n_dev, int shift0,
+                                                       int passes, unsigned *ghist) {
+    __shared__ unsigned h[SORT_MAX_PASSES][256];
     const int n = n_dev ? *n_dev : n_host;
-    h[threadIdx.x] = 0;
+    for (int k = threadIdx.x; k < SORT_MAX_PASSES * 256; k += 256) (&h[0][0])[k] = 0;
     __syncthreads();
-    i64 base = (i64)blockIdx.x * SORT_TILE;
-    for (int j = 0; j < SORT_ITEMS; ++j) {
-        i64 i = base + j * SORT_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&h[(unsigned)(kin[i] >> shift) & 255u], 1u);
+    for (i64 i = (i64)blockIdx.x * 256 + threadIdx.x; i < n; i += (i64)gridDim.x * 256) {
+        const u64 key = kin[i] >> shift0;
+        for (int p = 0; p < passes; ++p) atomicAdd(&h[p][(unsigned)(key >> (8 * p)) & 255u], 1u);
     }
     __syncthreads();
-    hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+    for (int p = 0; p < passes; ++p) {
+        const unsigned c = h[p][threadIdx.x];
+        if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c);
+    }
+}
+
+// exclusive scan of the 256 counts of every pass, in place (one block, thread = digit)
+__global__ void __launch_bounds__(256) k_sort_bases(unsigned *ghist, int passes) {
+    __shared__ unsigned wsum[8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int p = 0; p < passes; ++p) {
+        const unsigned c = ghist[p * 256 + threadIdx.x];
+        unsigned inc = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+        if (lane == 31) wsum[w] = inc;
+        __syncthreads();
+        unsigned off = 0;
+        for (int k = 0; k < w; ++k) off += wsum[k];
+        ghist[p * 256 + threadIdx.x] = off + inc - c;
+        __syncthreads();
+    }
 }
 
 // Stable scatter of one 8-bit digit.  Ranks inside a warp come from match_any; the tile is first
@@ -160,25 +201,28 @@ struct SortSmem {
 };
 
 __global__ void __launch_bounds__(SORT_THREADS)
-k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__restrict__ kout,
-               int *__restrict__ vout, int n_host, const int *n_dev, int shift,
-               const unsigned *__restrict__ offs, int nblocks) {
+k_sort_pass(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__restrict__ kout,
+            int *__restrict__ vout, int n_host, const int *n_dev, int shift,
+            const unsigned *__restrict__ base, unsigned *state, unsigned *ticket) {
     extern __shared__ __align__(16) unsigned char sort_raw[];
     SortSmem &sm = *reinterpret_cast<SortSmem *>(sort_raw);
+    __shared__ int s_tile;
     const int n = n_dev ? *n_dev : n_host;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
     for (int k = threadIdx.x; k < SORT_WARPS * 256; k += SORT_THREADS) (&sm.wc[0][0])[k] = 0;
-    sm.gbase[threadIdx.x] = offs[threadIdx.x * nblocks + blockIdx.x];
     __syncthreads();
-    const i64 tile0 = (i64)blockIdx.x * SORT_TILE;
-    const i64 base = tile0 + (i64)w * (32 * SORT_ITEMS);
+    const int tile = s_tile;
+    const i64 tile0 = (i64)tile * SORT_TILE;
+    if (tile0 >= n) return;                                     // (tiles beyond a device-side n: nobody looks at them)
+    const i64 wbase = tile0 + (i64)w * (32 * SORT_ITEMS);
     u64 key[SORT_ITEMS];
     int val[SORT_ITEMS];
     unsigned rank[SORT_ITEMS];
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
     for (int j = 0; j < SORT_ITEMS; ++j) {
-        i64 i = base + j * 32 + lane;
+        i64 i = wbase + j * 32 + lane;
         bool valid = i < n;
         key[j] = valid ? kin[i] : 0ull;
         val[j] = valid ? vin[i] : 0;
@@ -192,12 +236,44 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
     }
     __syncthreads();
     unsigned tot;
-    {   // exclusive scan over warps, one digit per thread; then over the digits of the tile
+    {   // exclusive scan over warps, one digit per thread
         unsigned run = 0;
         for (int k = 0; k < SORT_WARPS; ++k) { unsigned t = sm.wc[k][threadIdx.x]; sm.wc[k][threadIdx.x] = run; run += t; }
         tot = run;
     }
-    {
+    {   // equal digits in all earlier tiles: publish, look back, publish the inclusive prefix
+        cuda::atomic_ref<unsigned, cuda::thread_scope_device> mine(state[(size_t)tile * 256 + threadIdx.x]);
+        unsigned excl = 0;
+        if (tile == 0) mine.store(SORT_FLAG_P | tot, cuda::std::memory_order_relaxed);
+        else {
+            mine.store(SORT_FLAG_A | tot, cuda::std::memory_order_relaxed);
+            // a window of SORT_LOOK predecessors is read at once (independent loads), then consumed in order
+            int t = tile - 1;
+            bool done = false;
+            while (!done) {
+                unsigned v[SORT_LOOK];
+#pragma unroll
+                for (int q = 0; q < SORT_LOOK; ++q) {
+                    cuda::atomic_ref<unsigned, cuda::thread_scope_device> prev(state[(size_t)max(t - q, 0) * 256 + threadIdx.x]);
+                    v[q] = prev.load(cuda::std::memory_order_relaxed);
+                }
+                int used = 0;
+#pragma unroll
+                for (int q = 0; q < SORT_LOOK; ++q) {
+                    if (!done && used == q && (v[q] >> 30) != 0u) {      // ready, and everything nearer was ready too
+                        excl += v[q] & SORT_CNT_MASK;
+                        ++used;
+                        if (v[q] & SORT_FLAG_P) done = true;          // (tile 0 always ends the walk: t - q >= 0 here)
+                    }
+                }
+                t -= used;
+                if (used == 0) __nanosleep(20);
+            }
+            mine.store(SORT_FLAG_P | (excl + tot), cuda::std::memory_order_relaxed);
+        }
+        sm.gbase[threadIdx.x] = base[threadIdx.x] + excl;
+    }
+    {   // start of every digit inside the tile
         unsigned inc = tot;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
@@ -211,7 +287,7 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < SORT_ITEMS; ++j) {
-        i64 i = base + j * 32 + lane;
+        i64 i = wbase + j * 32 + lane;
         if (i < n) {
             unsigned dg = (unsigned)(key[j] >> shift) & 255u;
             unsigned lp = sm.lstart[dg] + sm.wc[w][dg] + rank[j];
@@ -232,20 +308,23 @@ k_sort_scatter(const u64 *__restrict__ kin, const int *__restrict__ vin, u64 *__
 
 // one-time kernel attributes (called by sph_create, outside any stream capture)
 void sph_sort_init() {
-    cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    cudaFuncSetAttribute(k_sort_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
 }
 
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur) {
     const int nblocks = sph_ceil_div(n_host, SORT_TILE);
+    const int passes = (bits + 7) / 8;
+    unsigned *ws = ctx->d.hist, *ticket = ws, *ghist = ws + 64, *state = ws + 64 + SORT_MAX_PASSES * 256;
+    cudaMemsetAsync(ws, 0, (64 + SORT_MAX_PASSES * 256 + (size_t)passes * 256 * nblocks) * sizeof(unsigned), ctx->stream);
     int c = *cur;
-    for (int shift = 0; shift < bits; shift += 8) {
-        k_sort_hist<<<nblocks, 256, 0, ctx->stream>>>(key[c], n_host, n_dev, shift, ctx->d.hist, nblocks);
-        sph_scan_u32(ctx, ctx->d.hist, ctx->d.hist, (i64)256 * nblocks, (unsigned *)ctx->d.scan_tmp);
-        k_sort_scatter<<<nblocks, SORT_THREADS, sizeof(SortSmem), ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host,
-                                                                  n_dev, shift, ctx->d.hist, nblocks);
-        ctx->launches += 2;
+    k_sort_hist_all<<<min(sph_ceil_div(n_host, 2048), 148 * 8), 256, 0, ctx->stream>>>(key[c], n_host, n_dev, 0, passes, ghist);
+    k_sort_bases<<<1, 256, 0, ctx->stream>>>(ghist, passes);
+    for (int p = 0; p < passes; ++p) {
+        k_sort_pass<<<nblocks, SORT_THREADS, sizeof(SortSmem), ctx->stream>>>(key[c], val[c], key[c ^ 1], val[c ^ 1], n_host, n_dev, 8 * p,
+                                                                 ghist + p * 256, state + (size_t)p * 256 * nblocks, ticket + p);
         c ^= 1;
     }
+    ctx->launches += 2 + passes;
     *cur = c;
 }
 

@@ -197,6 +197,7 @@ static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 // Result ends in key[*cur], val[*cur].
 void sph_radix_sort(sph_ctx *ctx, u64 *key[2], int *val[2], int n_host, const int *n_dev, int bits, int *cur);
 void sph_sort_init();
+size_t sph_sort_ws_words(i64 n);   // words of Dev::hist the sort needs for n keys
 
 // ---- scan.cu ---- exclusive prefix sums (in == out allowed); scratch[ceil(n/2048)] = grand total
 void sph_scan_u32(sph_ctx *ctx, const unsigned *in, unsigned *out, i64 n, unsigned *scratch);
