@@ -189,12 +189,15 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     ms_dev = timed_steps()
     clocks = sampler.stop()
     launches = ctx.launch_count() - launches0
-    ctx.timing_enable(True)                  # region B: stage brackets and the walk's work counters (about 4 % of the walk)
-    ctx.counters_enable(True)
+    ctx.timing_enable(True)                  # region B: stage brackets around the kernels of the timed region
     ctx.timing_read()
     ms_bracketed = timed_steps()
     stages = ctx.timing_read()
     ctx.timing_enable(False)
+    # the algorithmic units of the rooflines: one more step, untimed, with the walk's work counters on (the counting
+    # variant of the walk is 15 % slower and is not the kernel the brackets time)
+    ctx.counters_enable(True)
+    ctx.step(w.dt)
     counters = ctx.get_counters()
     ctx.counters_enable(False)
     out = dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters,
