@@ -816,7 +816,7 @@ static int step_enqueue(sph_ctx *ctx, double dt) {
     return check_cuda(ctx, "sph_step");
 }
 
-// A step is ~170 launches; for the small workloads (C1-C3) the GPU idles between them.  The launch
+// A step is ~80 launches; for the small workloads (C1-C3) the GPU idles between them.  The launch
 // sequence of a step depends only on the configuration and on dt, so it is captured into a CUDA
 // graph the second time in a row a dt is asked for and replayed from then on (stage timing runs the
 // plain launches: event brackets are not part of the graph).
