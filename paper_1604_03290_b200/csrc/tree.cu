@@ -162,127 +162,93 @@ __device__ __forceinline__ void cell_moments(const Dev &d, int nd, bool hmax_onl
     }
 }
 
-// Bottom-up in ONE launch (the first version launched once per level: 21 launches, 0.75 ms on C5).
-// 2^D lanes own a cell, one child each: the children (cells or single particles) are loaded side by side, the masses and
-// the mass-weighted positions are then added in octant order -- every lane runs the same chain on values fetched with
-// shuffles, so the arithmetic is that of cell_moments, bit for bit -- and boxes and hmax are reduced by a butterfly
-// (min and max do not depend on the order).  A leaf of several particles sends the cell to cell_moments (its particles
-// enter the chain one by one).  The group starts at a cell without child cells and climbs: after finishing a cell its
-// first lane increments the parent's counter; the group that brings the counter to the parent's number of child
-// cells computes the parent (all its children are complete and visible: release / acquire on the counter), the others
-// retire.  (One thread per cell with a serial loop over the children took 0.45 ms on C5, bound by the latency of
-// its dependent loads; profiles/r2_c5.md.)
-template <int D>
-__global__ void __launch_bounds__(256) k_moments(Dev d, int hmax_only) {
-    constexpr int NC = 1 << D, GPW = 32 / NC;                  // lanes per cell, cells per warp
-    const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31, c = lane % NC;
-    const int nn = d.status->n_nodes;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
-    for (int s0 = warp * GPW; s0 < nn; s0 += nwarps * GPW) {    // (uniform per warp)
-        const int slot = s0 + lane / NC;
-        int nd = (slot < nn && d.ncc[slot] == 0) ? slot : -1;
-        while (__any_sync(FULL, nd >= 0)) {
-            // ---- my child ----
-            double w = 0.0, q[3] = {0.0, 0.0, 0.0};
-            double mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY}, hm = 0.0;
-            int ex = 0;
-            bool multi = false;
-            if (nd >= 0) {
-                const int code = d.child[(size_t)nd * NC + c];
-                if (code >= 0) {                                // a cell finished earlier in this launch, by other threads
-                    ex = 1;
-                    hm = __ldcg(&d.nhmax[code]);
-                    if (!hmax_only) {
-                        w = __ldcg(&d.nmass[code]);
+// cell_moments with the loads of four children in flight at once (the serial form waits for one child after the
+// other: the launch was bound by the latency of those loads, 0.45 ms on C5).  The sums run in the same order on the same
+// values: same bits.  Returns false, with nothing written, when a leaf of several particles is among the children
+// (the caller then takes cell_moments).
+template <int D, bool HONLY>
+__device__ __forceinline__ bool cell_moments_batched(const Dev &d, int nd) {
+    constexpr int NC = 1 << D, HB = (NC < 4) ? NC : 4;
+    const int *cl = d.child_lo + (size_t)nd * (NC + 1);
+    const int *ch = d.child + (size_t)nd * NC;
+    int code[NC], lo[NC + 1];
 #pragma unroll
-                        for (int a = 0; a < D; ++a) {
-                            q[a] = __dmul_rn(w, __ldcg(&d.ncom[a][code]));
-                            mn[a] = __ldcg(&d.nbmin[a][code]);
-                            mx[a] = __ldcg(&d.nbmax[a][code]);
-                        }
-                    }
-                } else if (code == -2) {
-                    const int *cl = d.child_lo + (size_t)nd * (NC + 1) + c;
-                    const int p = cl[0];
-                    if (cl[1] - p == 1) {
-                        ex = 1;
-                        hm = d.sh[p];
-                        if (!hmax_only) {
-                            w = d.sm[p];
+    for (int c = 0; c < NC; ++c) { code[c] = ch[c]; lo[c] = cl[c]; }
+    lo[NC] = cl[NC];
 #pragma unroll
-                            for (int a = 0; a < D; ++a) {
-                                const double xp = d.sx[a][p];
-                                q[a] = __dmul_rn(w, xp);
-                                mn[a] = xp; mx[a] = xp;
-                            }
-                        }
-                    } else multi = true;
-                }
-            }
-            const unsigned gm = ((NC == 32) ? FULL : ((1u << NC) - 1u)) << (lane - c);
-            const bool serial = (__ballot_sync(FULL, multi) & gm) != 0u;   // a leaf of several particles among the children
-            // ---- masses and mass-weighted positions in octant order (reading U15) ----
-            double M = 0.0, S[3] = {0.0, 0.0, 0.0};
+    for (int c = 0; c < NC; ++c)
+        if (code[c] == -2 && lo[c + 1] - lo[c] != 1) return false;
+    double M = 0.0, S[3] = {0, 0, 0};
+    double bmin[3] = {INFINITY, INFINITY, INFINITY}, bmax[3] = {-INFINITY, -INFINITY, -INFINITY}, hmax = 0.0;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) {
-                const int exk = __shfl_sync(FULL, ex, k, NC);
-                const double wk = __shfl_sync(FULL, w, k, NC);
-                double qk[3];
+    for (int c0 = 0; c0 < NC; c0 += HB) {
+        double w[HB], hm[HB], x[HB][3], mn[HB][3], mx[HB][3];
 #pragma unroll
-                for (int a = 0; a < D; ++a) qk[a] = __shfl_sync(FULL, q[a], k, NC);
-                if (exk) {
-                    M = __dadd_rn(M, wk);
+        for (int k = 0; k < HB; ++k) {                        // all loads of the batch first
+            const int cd = code[c0 + k];
+            w[k] = 0.0; hm[k] = 0.0;
 #pragma unroll
-                    for (int a = 0; a < D; ++a) S[a] = __dadd_rn(S[a], qk[a]);
-                }
-            }
+            for (int a = 0; a < 3; ++a) { x[k][a] = 0.0; mn[k][a] = INFINITY; mx[k][a] = -INFINITY; }
+            if (cd >= 0) {
+                hm[k] = __ldcg(&d.nhmax[cd]);
+                if (!HONLY) {
+                    w[k] = __ldcg(&d.nmass[cd]);
 #pragma unroll
-            for (int o = 1; o < NC; o <<= 1) {
-                hm = fmax(hm, __shfl_xor_sync(FULL, hm, o, NC));
-#pragma unroll
-                for (int a = 0; a < D; ++a) {
-                    mn[a] = fmin(mn[a], __shfl_xor_sync(FULL, mn[a], o, NC));
-                    mx[a] = fmax(mx[a], __shfl_xor_sync(FULL, mx[a], o, NC));
-                }
-            }
-            int next = -1;
-            if (nd >= 0 && c == 0) {
-                if (serial) cell_moments(d, nd, hmax_only != 0);
-                else {
-                    d.nhmax[nd] = hm;
-                    if (!hmax_only) {
-                        d.nmass[nd] = M;
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) {
-                            d.ncom[a][nd] = (a < D) ? __ddiv_rn(S[a < D ? a : 0], M) : 0.0;
-                            d.nbmin[a][nd] = (a < D) ? mn[a < D ? a : 0] : 0.0;
-                            d.nbmax[a][nd] = (a < D) ? mx[a < D ? a : 0] : 0.0;
-                        }
+                    for (int a = 0; a < D; ++a) {
+                        x[k][a] = __ldcg(&d.ncom[a][cd]);
+                        mn[k][a] = __ldcg(&d.nbmin[a][cd]);
+                        mx[k][a] = __ldcg(&d.nbmax[a][cd]);
                     }
                 }
-                const int parent = d.nparent[nd];
-                if (parent >= 0) {
-                    // release my cell, acquire the siblings' cells: one acq_rel read-modify-write at device scope
-                    cuda::atomic_ref<int, cuda::thread_scope_device> ready(d.nready[parent]);
-                    const int done = ready.fetch_add(1, cuda::std::memory_order_acq_rel) + 1;
-                    if (done == d.ncc[parent]) next = parent;
+            } else if (cd == -2) {
+                const int p = lo[c0 + k];
+                hm[k] = d.sh[p];
+                if (!HONLY) {
+                    w[k] = d.sm[p];
+#pragma unroll
+                    for (int a = 0; a < D; ++a) { x[k][a] = d.sx[a][p]; mn[k][a] = x[k][a]; mx[k][a] = x[k][a]; }
                 }
             }
-            nd = __shfl_sync(FULL, next, 0, NC);                // the group follows its first lane
-            __syncwarp();                                       // ... whose acquire orders the loads of all its lanes
+        }
+#pragma unroll
+        for (int k = 0; k < HB; ++k) {                        // then the sums, in octant order
+            if (code[c0 + k] == -1) continue;
+            hmax = fmax(hmax, hm[k]);
+            if (HONLY) continue;
+            M = __dadd_rn(M, w[k]);
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+                S[a] = __dadd_rn(S[a], __dmul_rn(w[k], x[k][a]));
+                bmin[a] = fmin(bmin[a], mn[k][a]);
+                bmax[a] = fmax(bmax[a], mx[k][a]);
+            }
         }
     }
+    d.nhmax[nd] = hmax;
+    if (HONLY) return true;
+    d.nmass[nd] = M;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        d.ncom[a][nd] = (a < D) ? __ddiv_rn(S[a < D ? a : 0], M) : 0.0;
+        d.nbmin[a][nd] = (a < D) ? bmin[a < D ? a : 0] : 0.0;
+        d.nbmax[a][nd] = (a < D) ? bmax[a < D ? a : 0] : 0.0;
+    }
+    return true;
 }
 
-// One thread per cell, serial over the children: the widest form (every cell without child cells starts at once), best
-// for large sets where the launch is bound by memory throughput.
-__global__ void k_moments_wide(Dev d, int hmax_only) {
+// Bottom-up in ONE launch (the first version launched once per level: 21 launches, 0.75 ms on C5).  A thread starts at
+// a cell without child cells and climbs: after finishing a cell it increments the parent's counter; the thread that
+// brings the counter to the parent's number of child cells computes the parent (all its children are complete and
+// visible: release / acquire on the counter), the others retire.  The arithmetic of a cell does not depend on which
+// thread performs it.  (2^D lanes per cell with the ordered sums done by shuffles were measured too: faster than the
+// serial loop over the children for small sets, slower than the batched loads everywhere; profiles/r2_c5.md.)
+template <int D, bool HONLY>
+__global__ void k_moments(Dev d) {
     int nd = blockIdx.x * blockDim.x + threadIdx.x;
     if (nd >= d.status->n_nodes) return;
     if (d.ncc[nd] != 0) return;
     while (true) {
-        cell_moments(d, nd, hmax_only != 0);
+        if (!cell_moments_batched<D, HONLY>(d, nd)) cell_moments(d, nd, HONLY);
         const int parent = d.nparent[nd];
         if (parent < 0) return;
         // release my cell, acquire the siblings' cells: one acq_rel read-modify-write at device scope
@@ -293,7 +259,6 @@ __global__ void k_moments_wide(Dev d, int hmax_only) {
     }
 }
 
-#define MOMENTS_WIDE_FROM 500000
 __global__ void k_reset_ready(Dev d) {
     const int nd = blockIdx.x * blockDim.x + threadIdx.x;
     if (nd < d.status->n_nodes) d.nready[nd] = 0;
@@ -305,11 +270,9 @@ void sph_launch_moments(sph_ctx *ctx, int hmax_only) {
         k_reset_ready<<<sph_ceil_div(d.n, 256), 256, 0, ctx->stream>>>(d);
         ctx->launches += 1;
     }
-    // measured (profiles/r2_c5.md): groups of lanes 2-3x faster up to 0.4 M particles (C1 59 -> 25 us, C2 138 -> 43, C6 118 -> 61),
-    // equal at 0.5 M (C3), one thread per cell faster beyond (C4 253 against 337 us, C5 448 against 849)
-    if (d.n > MOMENTS_WIDE_FROM) k_moments_wide<<<sph_ceil_div(d.n, 128), 128, 0, ctx->stream>>>(d, hmax_only);
-    else if (d.D == 3) k_moments<3><<<148 * 8, 256, 0, ctx->stream>>>(d, hmax_only);   // the warps stride over the cells
-    else k_moments<2><<<148 * 8, 256, 0, ctx->stream>>>(d, hmax_only);
+    const int blocks = sph_ceil_div(d.n, 128);
+    if (d.D == 3) { if (hmax_only) k_moments<3, true><<<blocks, 128, 0, ctx->stream>>>(d); else k_moments<3, false><<<blocks, 128, 0, ctx->stream>>>(d); }
+    else { if (hmax_only) k_moments<2, true><<<blocks, 128, 0, ctx->stream>>>(d); else k_moments<2, false><<<blocks, 128, 0, ctx->stream>>>(d); }
     ctx->launches += 1;
 }
 
