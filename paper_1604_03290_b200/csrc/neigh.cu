@@ -11,7 +11,7 @@
 //     bounding box and the largest h of the particles below it, rounded OUTWARD to FP32: pruning
 //     runs on the FP32 pipe with directed rounding (a box that holds a partner is never cut), the FP64
 //     pipe is kept for the exact membership tests.
-//   * Descent: lane = item.  A round takes the children of one cell from a small stack of ranges; every
+//   * Descent: lane = item.  A round takes the children of up to four cells from a small stack of ranges; every
 //     lane tests ITS item against the bounding box of the whole group (one test per item, not one per
 //     item and particle) and cells within reach push their children.
 //   * Buckets within reach of the group box are then looked at by lane = particle: every lane tests
@@ -33,7 +33,11 @@
 #include "sph_internal.cuh"
 
 #define NB_WARPS 2
-#define NB_STACK 192            // ranges of child items per warp: <= 8 pending siblings per tree level
+#define NB_STACK 384            // ranges of child items per warp
+#define NB_RESERVE 168          // a depth-first descent keeps <= 8 pending siblings per tree level (21 levels)
+#ifndef NB_RANGES
+#define NB_RANGES 4             // ranges (cells) whose child items one round tests
+#endif
 
 // ------------------------------------------------------------------------------------------
 // search tree
@@ -230,13 +234,35 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     if (lane == 0) { const int2 root = __ldg(reinterpret_cast<const int2 *>(reinterpret_cast<const float4 *>(items) + 2)); stack[0] = root; }
     __syncwarp();
     while (top > 0) {
-        // ---- lane = item: the children of one cell against the box of the group ----
-        const int2 rg = stack[top - 1];                       // first child item, number of child items
-        const int take = min(32, rg.y);
-        __syncwarp();
-        if (rg.y > 32) { if (lane == 0) stack[top - 1] = make_int2(rg.x + 32, rg.y - 32); }
-        else --top;
-        const int it = rg.x + min(lane, take - 1);
+        // ---- lane = item: the children of up to NB_RANGES cells against the box of the group ----
+        // (a cell has at most 2^D child items, so one range fills a quarter of the warp: several ranges per round while the
+        // stack has room for the ranges their cells may push, one range -- a plain depth-first descent -- otherwise)
+        int it = 0, take = 0;
+        {
+            const int nrmax = (top + 32 <= NB_STACK - NB_RESERVE) ? NB_RANGES : 1;
+            int2 rgs[NB_RANGES];
+            int nr = 0;
+#pragma unroll
+            for (int r = 0; r < NB_RANGES; ++r) {
+                rgs[r] = make_int2(0, 0);
+                if (r < nrmax && top - r > 0) rgs[r] = stack[top - 1 - r];
+            }
+            __syncwarp();
+            int newtop = top;
+#pragma unroll
+            for (int r = 0; r < NB_RANGES; ++r) {
+                if (rgs[r].y > 0 && take < 32 && nr == r) {
+                    const int tk = min(32 - take, rgs[r].y);
+                    if (lane >= take && lane < take + tk) it = rgs[r].x + (lane - take);
+                    take += tk;
+                    if (tk < rgs[r].y) { if (lane == 0) stack[top - 1 - r] = make_int2(rgs[r].x + tk, rgs[r].y - tk); }   // the rest stays (it is the top entry then)
+                    else --newtop;
+                    ++nr;
+                }
+            }
+            top = newtop;
+            __syncwarp();
+        }
         const float4 *rec = reinterpret_cast<const float4 *>(items + it);
         const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);            // bmin xyz bmax x | bmax yz hmax pad
         const int2 ab = __ldg(reinterpret_cast<const int2 *>(rec + 2));
@@ -270,7 +296,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
         while (buckets) {
             const int src = __ffs(buckets) - 1;
             buckets &= buckets - 1;
-            const float4 *brec = reinterpret_cast<const float4 *>(items + rg.x + src);
+            const float4 *brec = reinterpret_cast<const float4 *>(items + __shfl_sync(FULL, it, src));
             const float4 b0 = __ldg(brec), b1 = __ldg(brec + 1);
             const int2 bl = __ldg(reinterpret_cast<const int2 *>(brec + 2));
             const int m = -bl.x, lo = bl.y;
