@@ -29,6 +29,7 @@
 // Lists are written group-transposed, nb[(group*cap + k)*32 + lane], so that the pair-sum kernel
 // reads them fully coalesced.
 #include <algorithm>
+#include <type_traits>
 
 #include "sph_internal.cuh"
 
@@ -190,6 +191,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     const double xi = d.sx[0][ii], yi = d.sx[1][ii], zi = (D == 3) ? d.sx[2][ii] : 0.0;
     const double Hi = d.sh[ii];
     const double Hi2 = __dmul_rn(Hi, Hi);
+    const double xq = valid ? xi : __longlong_as_double(0x7ff8000000000000ll);   // membership tests of a tail lane compare NaN: never a partner
     constexpr bool VH = VARH && !COUNT_ONLY;   // pair criterion (h_a + h_b)/2, eq. 72
     const float xlo = __double2float_rd(xi), xhi = __double2float_ru(xi), ylo = __double2float_rd(yi), yhi = __double2float_ru(yi);
     const float zlo = __double2float_rd(zi), zhi = __double2float_ru(zi);
@@ -319,21 +321,45 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
                 if (VARH && !COUNT_ONLY) s_c[w][3][lane] = d.sh[p];
             }
             __syncwarp();
-            for (int j = 0; j < m; ++j) {
-                const double dx = __dsub_rn(xi, s_c[w][0][j]);
-                const double dy = __dsub_rn(yi, s_c[w][1][j]);
-                const double dz = (D == 3) ? __dsub_rn(zi, s_c[w][2][j]) : 0.0;
-                const double r2 = sph_r2_exact(dx, dy, dz, D);
-                double H2 = Hi2;
-                if (VARH && !COUNT_ONLY) {
-                    const double Hab = __dmul_rn(0.5, __dadd_rn(Hi, s_c[w][3][j]));
-                    H2 = __dmul_rn(Hab, Hab);
+            // The exact test of every member, a predicated store and a predicated count per member (no branch).  Two things
+            // are settled per bucket instead of per member: whether the bucket holds a particle of the group (only then a
+            // member can be the lane's own particle) and whether every lane has room for all members (only otherwise the
+            // capacity is checked per store).
+            const int jself = i - lo;
+            const bool own = __any_sync(FULL, (unsigned)jself < (unsigned)m);
+            const bool tight = __any_sync(FULL, cnt + m > cap);
+            auto members = [&](auto own_c, auto tight_c) {
+                constexpr bool OWN = decltype(own_c)::value, TIGHT = decltype(tight_c)::value;
+#pragma unroll 4
+                for (int j = 0; j < m; ++j) {
+                    const double dx = __dsub_rn(xq, s_c[w][0][j]);
+                    const double dy = __dsub_rn(yi, s_c[w][1][j]);
+                    const double dz = (D == 3) ? __dsub_rn(zi, s_c[w][2][j]) : 0.0;
+                    const double r2 = sph_r2_exact(dx, dy, dz, D);
+                    double H2 = Hi2;
+                    if (VARH && !COUNT_ONLY) {
+                        const double Hab = __dmul_rn(0.5, __dadd_rn(Hi, s_c[w][3][j]));
+                        H2 = __dmul_rn(Hab, Hab);
+                    }
+                    if (TIGHT || COUNT_ONLY) {
+                        const bool hit = (!OWN || j != jself) && r2 < H2;      // (a lane beyond the slice compares NaN: never a hit)
+                        if (!COUNT_ONLY && hit && cnt < cap) nbw[(size_t)cnt * 32] = lo + j;
+                        cnt += hit ? 1 : 0;
+                    } else if (OWN) {
+                        // compare, store and count under ONE predicate
+                        asm volatile("{ .reg .pred p, q; setp.ne.s32 q, %5, %6; setp.lt.and.f64 p, %3, %4, q;\n"
+                                     "  @p st.global.s32 [%1], %2; @p add.s32 %0, %0, 1; }"
+                                     : "+r"(cnt) : "l"(nbw + (size_t)cnt * 32), "r"(lo + j), "d"(r2), "d"(H2), "r"(jself), "r"(j) : "memory");
+                    } else {
+                        asm volatile("{ .reg .pred p; setp.lt.f64 p, %3, %4;\n"
+                                     "  @p st.global.s32 [%1], %2; @p add.s32 %0, %0, 1; }"
+                                     : "+r"(cnt) : "l"(nbw + (size_t)cnt * 32), "r"(lo + j), "d"(r2), "d"(H2) : "memory");
+                    }
                 }
-                if (valid && (lo + j != i) && r2 < H2) {
-                    if (!COUNT_ONLY && cnt < cap) nbw[(size_t)cnt * 32] = lo + j;
-                    ++cnt;
-                }
-            }
+            };
+            if (!own && !tight) members(std::false_type{}, std::false_type{});
+            else if (!tight) members(std::true_type{}, std::false_type{});
+            else members(std::true_type{}, std::true_type{});
             __syncwarp();
         }
     }
