@@ -121,22 +121,24 @@ __global__ void k_emit_items(Dev d, const unsigned *kcnt, const unsigned *kfirst
             const int len = (int)(m0 & 0xffull), ord = (int)((m0 >> 8) & 0xffffffull), par = (int)(m0 >> 32);
             const bool have = lane < len;
             const int p = s0 + (have ? lane : 0);
-            double mn[3], mx[3], hm = have ? d.sh[p] : 0.0;
+            // rounded outward to FP32 BEFORE the reduction: rounding is monotone, so min / max of the rounded values are
+            // the rounded min / max, and FP32 min / max is one instruction where FP64 costs four
+            float mn[3], mx[3], hm = have ? __double2float_ru(d.sh[p]) : 0.0f;
             for (int a = 0; a < 3; ++a) {
                 const double x = (a < D) ? d.sx[a][p] : 0.0;
-                mn[a] = x; mx[a] = x;
+                mn[a] = __double2float_rd(x); mx[a] = __double2float_ru(x);
             }
             for (int o = 16; o > 0; o >>= 1) {
                 for (int a = 0; a < 3; ++a) {
-                    mn[a] = fmin(mn[a], __shfl_xor_sync(FULL, mn[a], o));
-                    mx[a] = fmax(mx[a], __shfl_xor_sync(FULL, mx[a], o));
+                    mn[a] = fminf(mn[a], __shfl_xor_sync(FULL, mn[a], o));
+                    mx[a] = fmaxf(mx[a], __shfl_xor_sync(FULL, mx[a], o));
                 }
-                hm = fmax(hm, __shfl_xor_sync(FULL, hm, o));
+                hm = fmaxf(hm, __shfl_xor_sync(FULL, hm, o));
             }
             if (lane == 0) {
                 SearchItem it;
-                for (int a = 0; a < 3; ++a) { it.bmin[a] = __double2float_rd(mn[a]); it.bmax[a] = __double2float_ru(mx[a]); }
-                it.hmax = __double2float_ru(hm); it.pad = 0.f; it.skip = -len; it.lo = s0; it.pad2[0] = it.pad2[1] = 0;
+                for (int a = 0; a < 3; ++a) { it.bmin[a] = mn[a]; it.bmax[a] = mx[a]; }
+                it.hmax = hm; it.pad = 0.f; it.skip = -len; it.lo = s0; it.pad2[0] = it.pad2[1] = 0;
                 d.items[1 + (int)kfirst[par] + ord] = it;
             }
         }
