@@ -1169,7 +1169,7 @@ int sph_get_neighbours(sph_ctx *ctx, int64_t *off, int32_t *idx, int64_t cap) {
                 const size_t i = g * 32 + lane;
                 if (i >= n) break;
                 int32_t *dst = idx + off[(size_t)perm[i]];
-                const int *src = buf.data() + (g - g0) * gcap + lane;
+                const int *src = buf.data() + (g - g0) * gcap + SPH_NB_POS(lane);
                 for (int k = 0; k < cnt[i]; ++k) dst[k] = perm[(size_t)src[(size_t)k * 32]];
                 std::sort(dst, dst + cnt[i]);
             }

@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
     // (an empty box B -- split = 31 -- has min = +big, max = -big: its distance to anything is huge)
 
     int cnt = 0;
-    int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
+    int *nbw = d.nb + (size_t)g * d.cap * 32 + SPH_NB_POS(lane);
     const int cap = d.cap;
     const SearchItem *__restrict__ items = d.items;
     int2 *stack = s_stack[w];
@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
         if (valid) d.nb_cnt[i] = min(cnt, cap);
         int mx = cnt;
         for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
+        for (int k = cnt; k < min(mx, cap); ++k) nbw[(size_t)k * 32] = ii;   // complete rows (SPH_NB_POS)
         int tot = valid ? min(cnt, cap) : 0;
         for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(FULL, tot, o);
         if (lane == 0) {

@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(128) k_density(Dev d) {
     const int cnt = valid ? d.nb_cnt[ii] : 0;
     int mx = cnt;
     for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    const int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
+    const int *nbw = d.nb + (size_t)g * d.cap * 32 + SPH_NB_POS(lane);
     const double iHi = 1.0 / Hi;
     double rho = d.sm[ii] * KNorm<D>::s * ((D == 3) ? iHi * iHi * iHi : iHi * iHi);   // self term (q = 0)
     for (int k = 0; k < mx; ++k) {
@@ -247,7 +247,8 @@ __global__ void __launch_bounds__(PR_WARPS * 32, PR_MINBLOCKS) k_pairs(Dev d, co
     const int cnt = valid ? d.nb_cnt[ii] : 0;
     int mx = cnt;
     for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
-    const int *nbw = d.nb + (size_t)g * d.cap * 32 + lane;
+    // the partner indices of the 8 rows my lane group stages (rows row0 + 4 t): 32 contiguous bytes per round (SPH_NB_POS)
+    const int4 *nbg = reinterpret_cast<const int4 *>(d.nb + (size_t)g * d.cap * 32 + (lane >> 3) * 8);
 
     double drho = 0.0, du = 0.0, dv[3] = {0, 0, 0};
     double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
@@ -261,24 +262,26 @@ __global__ void __launch_bounds__(PR_WARPS * 32, PR_MINBLOCKS) k_pairs(Dev d, co
 
     // copy the records of partners `b` (one per lane) into buffer `buf`
     const int sub = lane & 7, row0 = lane >> 3;
-    auto stage = [&](int b, int buf) {
+    auto stage = [&](int4 ia, int4 ib, int buf) {
         double *dstb = &s_buf[w][buf][0];
+        const int br[8] = {ia.x, ia.y, ia.z, ia.w, ib.x, ib.y, ib.z, ib.w};
 #pragma unroll
         for (int t = 0; t < 8; ++t) {
             const int r = row0 + 4 * t;
-            const int br = __shfl_sync(FULL, b, r);
-            cp_async16(dstb + r * PR_STRIDE + sub * 2, prec + (size_t)br * PR_REC + sub * 2);
+            cp_async16(dstb + r * PR_STRIDE + sub * 2, prec + (size_t)br[t] * PR_REC + sub * 2);
         }
     };
-    int b_next = (0 < cnt) ? nbw[0] : ii;
-    if (mx > 0) stage(b_next, 0);
+    // (rows k < mx are complete: a lane with fewer partners holds its own index there)
+    const int4 own4 = make_int4(ii, ii, ii, ii);
+    int4 ia = (mx > 0) ? __ldg(nbg) : own4, ib = (mx > 0) ? __ldg(nbg + 1) : own4;
+    if (mx > 0) stage(ia, ib, 0);
     cp_async_commit();
-    b_next = (1 < cnt) ? nbw[32] : ii;
+    if (mx > 1) { ia = __ldg(nbg + 8); ib = __ldg(nbg + 9); }
 
     for (int k = 0; k < mx; ++k) {
-        if (k + 1 < mx) stage(b_next, (k + 1) & 1);
+        if (k + 1 < mx) stage(ia, ib, (k + 1) & 1);
         cp_async_commit();
-        b_next = (k + 2 < cnt) ? nbw[(size_t)(k + 2) * 32] : ii;
+        if (k + 2 < mx) { ia = __ldg(nbg + (size_t)(k + 2) * 8); ib = __ldg(nbg + (size_t)(k + 2) * 8 + 1); }
         cp_async_wait1();
         __syncwarp();
         const double2 *rec = reinterpret_cast<const double2 *>(&s_buf[w][k & 1][lane * PR_STRIDE]);

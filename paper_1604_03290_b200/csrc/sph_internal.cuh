@@ -124,7 +124,7 @@ struct Dev {
     unsigned *bbox_done;        // blocks of k_bbox that have finished (0 between launches)
     u64 *bmark, *bscan;         // n+1 each: bucket starts (parent | ordinal | length); child-item counts and their scan
     u64 *scan_tmp;              // scratch of the prefix sums
-    // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + lane] (sorted indices) ----
+    // ---- partner lists: group-transposed, nb[(g*cap + k)*32 + SPH_NB_POS(lane)] (sorted indices) ----
     int *nb;
     int *nb_cnt;
     int *own_cnt;               // n_a of eq. 73
@@ -188,6 +188,12 @@ struct StageTimer {
     StageTimer(sph_ctx *ctx, int st) : c(ctx), stage(st) { if (c->timing) sph_timing_begin(c, stage); }
     ~StageTimer() { if (c->timing) sph_timing_end(c, stage); }
 };
+
+// Position of a lane's entry inside the 32 entries of a list row: lanes 0, 4, 8, ... 28 first, then 1, 5, ..., so that the
+// 8 lanes that stage one quarter of a row's records in the pair kernel (lanes r = q + 4 t) find their 8 partner indices in
+// 32 contiguous bytes.  Rows k < (largest count of the group) are complete: lanes with fewer partners hold their own
+// index there (a valid record that is read and ignored).
+#define SPH_NB_POS(lane) ((((lane) & 3) << 3) | ((lane) >> 2))
 
 static inline int sph_ceil_div(i64 a, i64 b) { return (int)((a + b - 1) / b); }
 
