@@ -292,6 +292,38 @@ int sph_measure_fp64_peak(void *cuda_stream, double *tflops);
  * scratch the caller provides (DEVICE src, dst). Synchronises. */
 int sph_measure_copy_bw(void *cuda_stream, const double *src, double *dst, size_t bytes, double *gbs);
 
+/* ---- Morton keys for callers that cannot allocate device memory (root cube eq. 67) ----
+ * Everything above needs a context, and a context needs a workspace the caller allocates.  A caller that has only the
+ * buffers it was given -- a plug-in inside a host application that owns the GPU memory pool, a time loop that must not
+ * pay the device-wide synchronisation of cudaMalloc / cudaFree, a process at its memory limit -- cannot get one.  This one
+ * call serves it: root cube and Morton keys (stages A1 of sph_build_tree, the same bits) with NO workspace argument.  It
+ * never calls cudaMalloc, cudaFree or any allocating routine: the scratch of the bounding-box reduction is a fixed array
+ * of SPH_STATIC_SCRATCH_BYTES inside the library's device image, which every GPU that loads the library holds until the
+ * process exits.
+ *
+ *   x, y, z   DEVICE, n doubles each, the caller's (z is ignored and may be NULL when dim == 2); read only.
+ *   n         1 .. SPH_STATIC_MAX_N; anything larger is rejected with SPH_ERR_ARG and a message (the kernels index with
+ *             int32 like the rest of the library, and the fixed scratch holds the partial boxes of at most 1024 blocks).
+ *   dim       2 or 3.   morton_bits   bits per dimension, 1..21; 0 = 21.
+ *   keys      DEVICE, n uint64, the caller's; keys[i] = key of particle i (ORIGINAL order, not sorted).
+ *   root      DEVICE double[4] or NULL: xmin, ymin, zmin (0 in 2-D) and the edge s0 of the root cube.
+ *   errbuf    HOST char[errbuf_len] or NULL: receives a one-line message when the call fails (empty on success).
+ * Asynchronous: two kernels and a 4-byte clear are enqueued on cuda_stream (a cudaStream_t, NULL = default stream); the
+ * buffers must stay valid until they have run.  Returns SPH_OK, SPH_ERR_ARG, or SPH_ERR_CUDA (no device, launch failure).
+ *
+ * Because the scratch is ONE array per GPU, shared by every call and every thread of the process:
+ *   - calls that can overlap on the GPU (streams with no ordering between them) race on it and produce wrong keys; keep the
+ *     calls on one stream or order them with events.  It shares nothing with contexts, so it may overlap with those;
+ *   - it keeps the last call's contents; the call clears the one word that has to start at zero (the arrival counter of
+ *     the reduction) on the stream before it launches, everything else is rewritten before it is read;
+ *   - the first call on a GPU looks up the array's device address (cudaGetSymbolAddress), which may load the library's
+ *     kernels onto that GPU: make that first call at set-up, with that GPU current on the calling thread, and before any
+ *     stream capture begins.  The GPU that is current must be the one the stream and the buffers belong to. */
+#define SPH_STATIC_MAX_N 0x3fffffff      /* 2^30 - 1 particles per call */
+#define SPH_STATIC_SCRATCH_BYTES 49408   /* device memory the library's image reserves on every GPU for this call */
+int sph_morton_keys_static(const double *x, const double *y, const double *z, int64_t n, int32_t dim, int32_t morton_bits,
+                           void *cuda_stream, uint64_t *keys, double *root, char *errbuf, size_t errbuf_len);
+
 const char *sph_last_error(sph_ctx *ctx);
 const char *sph_version(void);
 

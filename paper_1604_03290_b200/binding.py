@@ -24,8 +24,11 @@ EXPORTS = ["sph_workspace_bytes", "sph_create", "sph_destroy", "sph_upload", "sp
            "sph_find_neighbours", "sph_rhs", "sph_gravity", "sph_evaluate", "sph_step", "sph_step_host", "sph_download",
            "sph_sync", "sph_get_order", "sph_get_tree_size", "sph_get_tree", "sph_get_neighbours",
            "sph_launch_count", "sph_last_error", "sph_version", "sph_timing_enable", "sph_timing_read",
-           "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_partition", "sph_set_partition", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw"]
+           "sph_timing_name", "sph_get_counters", "sph_counters_enable", "sph_partition", "sph_set_partition", "sph_timestep", "sph_step_rk3", "sph_measure_fp64_peak", "sph_measure_copy_bw",
+           "sph_morton_keys_static"]
 SPH_T_COUNT = 11
+SPH_STATIC_MAX_N = 0x3FFFFFFF          # include/sph.h: largest n of sph_morton_keys_static
+SPH_STATIC_SCRATCH_BYTES = 49408
 
 # the caller's in-place all-gather (include/sph.h: sph_exchange_fn)
 EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_int32), C.c_int64)
@@ -114,6 +117,7 @@ def load_library():
     L.sph_step_rk3.argtypes = [_vp, C.c_double, C.c_double, _vp]
     L.sph_measure_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
     L.sph_measure_copy_bw.argtypes = [_vp, _vp, _vp, C.c_size_t, C.POINTER(C.c_double)]
+    L.sph_morton_keys_static.argtypes = [_vp, _vp, _vp, C.c_int64, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_char_p, C.c_size_t]
     _lib = L
     return L
 
@@ -492,3 +496,32 @@ def sph_measure_copy_bw(nbytes=1 << 30, stream=None):
     if rc != SPH_OK:
         raise SphError(rc, "sph_measure_copy_bw")
     return v.value
+
+
+def sph_morton_keys_static(x, y, z, keys, root=None, dim=3, morton_bits=21, stream=None):
+    """Root cube and Morton keys of the particles at (x, y, z) for a caller that cannot allocate device memory
+    (include/sph.h: sph_morton_keys_static): no context, no workspace; the library allocates nothing and uses its one
+    fixed scratch array per GPU, so calls that may overlap on the GPU must be ordered by the caller.
+
+    x, y, z: contiguous float64 CUDA tensors of equal length n (z may be None when dim == 2); keys: uint64 (or int64)
+    CUDA tensor of length n, written in the particles' ORIGINAL order; root: float64 CUDA tensor of length 4 or None.
+    Every buffer is the caller's: this wrapper, like the C call, creates none.  The work is enqueued on `stream`
+    (default: torch's current stream); n > SPH_STATIC_MAX_N raises SphError(SPH_ERR_ARG)."""
+    import torch
+    n = int(x.numel())
+    for t, dt in ((x, (torch.float64,)), (y, (torch.float64,)), (z, (torch.float64,)), (keys, (torch.uint64, torch.int64)),
+                  (root, (torch.float64,))):
+        if t is None:
+            continue
+        if not (t.is_cuda and t.is_contiguous() and t.dtype in dt and t.device == x.device):
+            raise SphError(SPH_ERR_ARG, "sph_morton_keys_static: contiguous CUDA tensors of one device, float64 / uint64")
+    if y.numel() != n or keys.numel() != n or (z is not None and z.numel() != n) or (root is not None and root.numel() != 4):
+        raise SphError(SPH_ERR_ARG, "sph_morton_keys_static: x, y, z, keys need one length, root needs 4 entries")
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(x.device):
+        st = stream if stream is not None else torch.cuda.current_stream(x.device)
+        rc = load_library().sph_morton_keys_static(
+            _vp(x.data_ptr()), _vp(y.data_ptr()), _vp(z.data_ptr()) if z is not None else None, n, dim, morton_bits,
+            _vp(st.cuda_stream), _vp(keys.data_ptr()), _vp(root.data_ptr()) if root is not None else None, err, len(err))
+    if rc != SPH_OK:
+        raise SphError(rc, err.value.decode())

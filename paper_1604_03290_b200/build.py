@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph_b200.so")
-SOURCES = ["api.cu", "order.cu", "tree.cu", "neigh.cu", "rhs.cu", "gravity.cu", "peak.cu", "scan.cu"]
+SOURCES = ["api.cu", "order.cu", "tree.cu", "neigh.cu", "rhs.cu", "gravity.cu", "peak.cu", "scan.cu", "static_keys.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--expt-relaxed-constexpr"]
 
