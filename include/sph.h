@@ -42,8 +42,9 @@ enum {
     SPH_ERR_STATE = -2,              /* call order: e.g. sph_rhs before sph_find_neighbours */
     SPH_ERR_WORKSPACE = -3,          /* workspace too small or misaligned (256 B) */
     SPH_ERR_NEIGHBOUR_OVERFLOW = -4, /* a particle has more than max_neighbours partners */
-    SPH_ERR_TREE_DEPTH = -5,         /* gravity walk: traversal stack exhausted (a guard: the pop policy bounds the stack for
-                                        every theta and particle distribution, see csrc/gravity.cu) */
+    SPH_ERR_TREE_DEPTH = -5,         /* a traversal stack was exhausted: the gravity walk's or the partner search's (guards: the
+                                        pop policies bound both stacks for every theta and particle distribution, see
+                                        csrc/gravity.cu and csrc/neigh.cu); sph_last_error names the kernel */
     SPH_ERR_CUDA = -6                /* CUDA runtime error or no device; see sph_last_error */
 };
 
@@ -227,7 +228,11 @@ int sph_download(sph_ctx *ctx, const sph_state_out *dst, int dst_is_device);
  * With SPH_F_DENSITY_SUM, or SPH_F_VARIABLE_H with h_iters > 0, the partner search and the density sum stay replicated
  * (every particle's density and smoothing length feed its partners' sums); the pair sums and the walk are still sharded.
  * sph_get_neighbours then returns the lists of the rank's own slice only; the work counters are per rank.  sph_step does
- * not capture CUDA graphs while a partition is set. */
+ * not capture CUDA graphs while a partition is set.
+ * The device-side failure flags (list overflow, stack guards, largest partner count) are collective: every exchange carries
+ * one more array of elem_bytes = 1 in which each rank's slot holds its flags, and after the all-gather every rank folds all
+ * slots into its own, so that all ranks return the same error from the same call and sph_step_rk3 accepts or gives back a
+ * step on all ranks alike.  The caller's exchange function needs no special case for it. */
 typedef int (*sph_exchange_fn)(void *user, void *cuda_stream, int n_arrays, void *const *arrays, const int32_t *elem_bytes,
                                int64_t slice_elems);
 int sph_partition(int64_t n, int world, int rank, int64_t *lo, int64_t *hi, int64_t *slice);
@@ -278,7 +283,7 @@ int sph_timing_enable(sph_ctx *ctx, int on);
 int sph_timing_read(sph_ctx *ctx, double *ms, int64_t *launches);
 const char *sph_timing_name(int stage);
 /* on != 0: the gravity walk also counts its interactions and opening tests (entries [2]-[4] of sph_get_counters;
- * about 4 % of the walk's time, so off by default; without it those entries read 0).  Drops a captured step graph. */
+ * the counting variant of the walk is about 15 % slower, so off by default; without it those entries read 0).  Drops a captured step graph. */
 int sph_counters_enable(sph_ctx *ctx, int on);
 /* Work counters of the LAST evaluation (HOST out[5]; synchronises): [0] internal nodes; [1] sum over
  * particles of the partner count; [2] sum over particles of gravity interactions (accepted pseudo-

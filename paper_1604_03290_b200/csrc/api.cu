@@ -112,8 +112,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     z.n_act_new = b.take<int>(np_);
     for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? np_ : 1);
     for (int k = 0; k < 9; ++k) { z.gradv[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); z.Cten[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); }
-    z.stage = b.take<double>(n);
-    z.stage_i = b.take<int>(n);
+    z.xstat = b.take<unsigned char>(np_);
     Mats *md = b.take<Mats>(1);
     if (mats_dev) *mats_dev = md;
     if (d) *d = z;
@@ -139,7 +138,9 @@ int status_flags(sph_ctx *ctx, const DevStatus &st, const char *where) {
         snprintf(ctx->err, sizeof(ctx->err), "interaction list overflow: %d partners > max_neighbours %d", st.nb_max, ctx->d.cap);
         return SPH_ERR_NEIGHBOUR_OVERFLOW;
     }
-    if (st.err_stack) return fail(ctx, SPH_ERR_TREE_DEPTH, "gravity walk: traversal stack exhausted (internal bound violated)");
+    if (st.err_stack)
+        return fail(ctx, SPH_ERR_TREE_DEPTH, (st.err_stack & 2) ? "partner search: descent stack exhausted (internal bound violated)"
+                                                                : "gravity walk: traversal stack exhausted (internal bound violated)");
     return check_cuda(ctx, where);
 }
 
@@ -184,6 +185,16 @@ void sph_timing_end(sph_ctx *ctx, int stage) {
 }
 
 static inline sph_ctx_ext *ext(sph_ctx *c) { return (sph_ctx_ext *)c; }
+
+// Dev::q0 holds the base copy of a step while one of the step calls is between its first and its last enqueue.  Host
+// downloads stage through q0 (sph_download), which stream order makes safe AFTER a step call has returned; a call that
+// arrived while the flag is up (a future split-step API, a second thread) would overwrite the base copy, so it is refused.
+struct Q0Live {
+    sph_ctx *c;
+    explicit Q0Live(sph_ctx *ctx) : c(ctx) { c->q0_live += 1; }
+    ~Q0Live() { c->q0_live -= 1; }
+};
+
 const sph_material *sph_dev_mats(sph_ctx *ctx) { return ext(ctx)->mats_dev->m; }
 
 // ------------------------------------------------------------------------------------------------
@@ -586,6 +597,7 @@ int sph_step_rk3(sph_ctx *ctx, double dt, double eps_des, double *out) {
     if (!ctx || !out) return SPH_ERR_ARG;
     if (!(ctx->d.flags & SPH_F_RK3)) return fail(ctx, SPH_ERR_STATE, "sph_step_rk3 needs SPH_F_RK3 at sph_create");
     if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step_rk3 before sph_upload");
+    Q0Live live(ctx);
     Dev &d = ctx->d;
     const size_t n = (size_t)d.n;
     const int gb = sph_ceil_div(d.n, 256);
@@ -677,6 +689,22 @@ int sph_set_partition(sph_ctx *ctx, int rank, int world, sph_exchange_fn fn, voi
     return SPH_OK;
 }
 
+// The failure flags steer control flow (sph_step_rk3 gives the state back, every synchronising call returns the error), so
+// they must be the same on every rank: a rank writes its three words (err_nb_overflow, err_stack, nb_max) into its slot of
+// a byte array that travels with the rates, and after the all-gather every rank folds all slots into its own status block
+// (OR, OR, max).  The flags are latched until the next upload, so folding them again later changes nothing.
+__global__ void k_status_pack(Dev d, int *slot) {
+    slot[0] = d.status->err_nb_overflow; slot[1] = d.status->err_stack; slot[2] = d.status->nb_max;
+}
+__global__ void k_status_merge(Dev d, const unsigned char *xstat, i64 slice, int world) {
+    int ov = 0, stk = 0, mx = 0;
+    for (int r = 0; r < world; ++r) {
+        const int *slot = reinterpret_cast<const int *>(xstat + (size_t)r * (size_t)slice);
+        ov |= slot[0]; stk |= slot[1]; mx = max(mx, slot[2]);
+    }
+    d.status->err_nb_overflow = ov; d.status->err_stack = stk; d.status->nb_max = mx;
+}
+
 // which: 1 = the arrays sph_rhs fills, 2 = the gravitational acceleration, 3 = both
 static int exchange_rates(sph_ctx *ctx, int which) {
     if (ctx->world <= 1 || !ctx->xfn) return SPH_OK;
@@ -685,6 +713,10 @@ static int exchange_rates(sph_ctx *ctx, int which) {
     int32_t eb[64];
     int na = 0;
     auto add = [&](void *p, int bytes) { arr[na] = p; eb[na] = bytes; ++na; };
+    // slice is a multiple of 32, so a slot of `slice` BYTES holds the three words and keeps them 4-byte aligned
+    k_status_pack<<<1, 1, 0, ctx->stream>>>(d, reinterpret_cast<int *>(d.xstat + (size_t)ctx->rank * (size_t)ctx->slice));
+    ctx->launches += 1;
+    add(d.xstat, 1);
     if (which & 1) {
         add(d.drho, 8); add(d.du, 8);
         // all components, also the zero rows of a 2-D run: every array a download can return is complete on every rank
@@ -696,9 +728,10 @@ static int exchange_rates(sph_ctx *ctx, int which) {
         add(d.nb_cnt, 4);
     }
     if ((which & 2) && (d.flags & SPH_F_GRAVITY)) for (int a = 0; a < 3; ++a) add(d.ag[a], 8);
-    if (na == 0) return SPH_OK;
     if (ctx->xfn(ctx->xuser, (void *)ctx->stream, na, arr, eb, (int64_t)ctx->slice) != 0)
         return fail(ctx, SPH_ERR_CUDA, "the caller's exchange function (all-gather of the rates) failed");
+    k_status_merge<<<1, 1, 0, ctx->stream>>>(d, d.xstat, ctx->slice, ctx->world);
+    ctx->launches += 1;
     return SPH_OK;
 }
 
@@ -823,6 +856,7 @@ static int step_enqueue(sph_ctx *ctx, double dt) {
 int sph_step(sph_ctx *ctx, double dt) {
     if (!ctx) return SPH_ERR_ARG;
     if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_step before sph_upload");
+    Q0Live live(ctx);
     if (ctx->timing || ctx->graphs_off || ctx->cfg.gravity_every > 1 || ctx->world > 1) return step_enqueue(ctx, dt);
     if (ctx->step_graph && ctx->graph_dt == dt) {
         if (cudaGraphLaunch(ctx->step_graph, ctx->stream) != cudaSuccess) return check_cuda(ctx, "sph_step (graph)");
@@ -923,6 +957,7 @@ static int host_step_enqueue(sph_ctx *ctx, const sph_state_in *s, double dt) {
 
 int sph_step_host(sph_ctx *ctx, const sph_state_in *s, double dt) {
     if (!ctx || !s) return SPH_ERR_ARG;
+    Q0Live live(ctx);
     // stage timing, decoupled gravity and sharded runs take the plain sequence
     if (ctx->timing || ctx->cfg.gravity_every > 1 || ctx->world > 1 || !ctx->copy_stream) {
         const int rc = sph_upload(ctx, s, 0);
@@ -980,6 +1015,8 @@ int sph_sync(sph_ctx *ctx) {
 int sph_download(sph_ctx *ctx, const sph_state_out *o, int dst_is_device) {
     if (!ctx || !o) return SPH_ERR_ARG;
     if (!ctx->have_state) return fail(ctx, SPH_ERR_STATE, "sph_download before sph_upload");
+    if (!dst_is_device && ctx->q0_live)
+        return fail(ctx, SPH_ERR_STATE, "sph_download to host buffers while a step call is under way (its base copy is the staging area)");
     Dev &d = ctx->d;
     const int n = d.n;
     const size_t nb = (size_t)n * 8;

@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32) k_neigh(Dev d) {
             if (pos < NB_STACK) stack[pos] = ab;
         }
         top += __popc(cells);
-        if (top > NB_STACK) { if (lane == 0) atomicExch(&d.status->err_stack, 1); break; }   // unreachable: <= 8 pending siblings per level
+        if (top > NB_STACK) { if (lane == 0) atomicOr(&d.status->err_stack, 2); break; }   // unreachable: <= 8 pending siblings per level
         __syncwarp();
         // ---- lane = particle: the admitted buckets, in Morton order ----
         while (buckets) {

@@ -20,7 +20,7 @@ typedef long long i64;
 struct DevStatus {
     int n_nodes;        // internal octree nodes found by the last build
     int err_nb_overflow;
-    int err_stack;
+    int err_stack;      // bit 0: the gravity walk's stack guard fired, bit 1: the partner search's
     int nb_max;         // largest partner count seen
     // work counters of the last evaluation (algorithmic units for the roofline)
     u64 n_pairs;        // sum over particles of |N(a)|               (A5)
@@ -136,9 +136,8 @@ struct Dev {
     double *dxs[3];             // XSPH term of eq. 40 (only with SPH_F_XSPH)
     double *gradv[9], *Cten[9]; // velocity gradient (eq. 42) and correction tensor (eq. 43), row-major (only with SPH_F_EXPORT_GRADV)
     int *n_act_new;
-    // ---- staging ----
-    double *stage;              // n doubles, for unsorting downloads
-    int *stage_i;               // n ints
+    // ---- sharding: the ranks' failure flags travel with the rates (api.cu exchange_rates) ----
+    unsigned char *xstat;       // world * slice bytes; rank r's slot = 3 ints at byte r * slice
 };
 
 struct SphTiming;   // api.cu: CUDA-event pairs around the stages (sph_timing_*)
@@ -160,6 +159,7 @@ struct sph_ctx {
     sph_exchange_fn xfn;
     void *xuser;
     int in_evaluate;
+    int q0_live;                // inside sph_step / sph_step_host / sph_step_rk3: Dev::q0 holds the base copy (no host download)
     int sort_cur;
     SphTiming *timing;          // NULL unless sph_timing_enable(ctx, 1)
     // sph_step as a CUDA graph: captured when the same dt is asked for twice in a row, replayed after

@@ -806,6 +806,48 @@ def test_sharded_evaluation_and_step_equal_single_gpu_bit_for_bit(P, name, world
     vr.close()
 
 
+def test_sharded_failure_flags_are_collective(P):
+    """the device-side failure flags steer control flow (every synchronising call returns them, sph_step_rk3
+    gives the state back), so on a sharded run they must agree on all ranks.  Here only rank 0's slice holds particles
+    with more partners than max_neighbours (a clump in the low-z half of the box): both ranks must return
+    SPH_ERR_NEIGHBOUR_OVERFLOW from the same calls, report the same largest count, and end sph_step_rk3 with the
+    state they started from."""
+    w = CASES["blob3d"]()
+    w.x[:, :60] = 0.25 + 0.004 * np.random.default_rng(99).standard_normal((3, 60))
+    w.flags |= P.SPH_F_RK3
+    cap, world = 112, 2
+    big = make_ctx(P, w, max_neighbours=256)
+    big.evaluate()
+    cnt = big.download(("nb_count",))["nb_count"]
+    _, perm, _ = big.get_order()
+    big.close()
+    lo1, _, _ = P.sph_partition(w.n, world, 1)
+    assert cnt[perm][:lo1].max() > cap >= cnt[perm][lo1:].max(), "the case must overflow in rank 0's slice only"
+
+    vr = VirtualRanks(P, w, world, max_neighbours=cap)
+
+    def job(ctx):
+        codes, msgs = [], []
+        ctx.evaluate()
+        for call in (ctx.sync, ctx.timestep, ctx.get_counters, lambda: ctx.step_rk3(w.dt, 1e30)):
+            try:
+                call()
+                codes.append(0)
+            except P.SphError as e:
+                codes.append(e.code)
+                msgs.append(str(e))
+        state = {k: v.cpu().numpy() for k, v in ctx.download(P.STATE_FIELDS, device=True).items()}
+        return codes, msgs, state
+
+    res = vr.run(job)
+    for r, (codes, msgs, state) in enumerate(res):
+        assert codes == [P.SPH_ERR_NEIGHBOUR_OVERFLOW] * 4, (r, codes)
+        assert all(f"{cnt.max()} partners" in m for m in msgs), (r, msgs)        # the largest count of ALL slices
+        for k, want in (("x", w.x), ("v", w.v), ("rho", w.rho), ("u", w.u), ("S", w.S), ("dmg", w.dmg), ("h", w.h)):
+            assert np.array_equal(state[k], want), (r, k)
+    vr.close()
+
+
 def test_nccl_all_gather_call_on_device_memory(P):
     """The binding's all-gather on CUDA memory through torch.distributed's NCCL backend, with the one rank this box
     has: checks the call itself (uint8 views over raw device pointers, in-place input/output aliasing, the library's
