@@ -189,17 +189,24 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     ms_dev = timed_steps()
     clocks = sampler.stop()
     launches = ctx.launch_count() - launches0
+    snap = ctx.download(P.STATE_FIELDS, device=True)      # the state region B starts from (device copy, untimed)
     ctx.timing_enable(True)                  # region B: stage brackets around the kernels of the timed region
     ctx.timing_read()
     ms_bracketed = timed_steps()
     stages = ctx.timing_read()
     ctx.timing_enable(False)
-    # the algorithmic units of the rooflines: one more step, untimed, with the walk's work counters on (the counting
-    # variant of the walk is 15 % slower and is not the kernel the brackets time)
+    # the algorithmic units of the rooflines, on the SAME states as the bracketed region: back to the snapshot, the same K
+    # steps once more, untimed, with the walk's work counters on (the counting variant of the walk is 15 % slower and is
+    # not the kernel the brackets time); the counters of a step are those of its second evaluation, averaged over the steps
+    ctx.upload(device=True, **snap)
     ctx.counters_enable(True)
-    ctx.step(w.dt)
-    counters = ctx.get_counters()
+    per_step = []
+    for _ in range(args.steps):
+        ctx.step(w.dt)
+        per_step.append(ctx.get_counters())
     ctx.counters_enable(False)
+    counters = {k: int(round(sum(c[k] for c in per_step) / len(per_step))) for k in per_step[0]}
+    del snap
     out = dict(w=w, ms_dev=ms_dev, ms_bracketed=ms_bracketed, launches=launches, stages=stages, counters=counters,
                clocks=clocks, l2_flush=small, ws_bytes=ws_bytes, t_gen=t_gen, n_own=hi - lo)
     if not full:
@@ -221,7 +228,7 @@ def measure_workload(P, torch, name, args, rank, world, dev, full):
     ctx.upload_workload(w)
 
     # ---- end-to-end arm: host buffers through the C ABI every step ----
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = max(1, args.steps)                          # the same K as the device-resident arm
     n = w.n
     pin = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=True)
     host = dict(x=pin((3, n), torch.float64), v=pin((3, n), torch.float64), rho=pin((n,), torch.float64),
@@ -479,7 +486,8 @@ def main():
     stages, roofs = stage_tables(r, evals, r["fp64_peak"], hbm_peak)
     top = max(stages, key=lambda k: stages[k]["share"])
     roofline = dict(roofs[top])
-    roofline.update({"kernel": top, "traffic": TRAFFIC_NCU.get((args.workload, top)),
+    roofline.update({"kernel": top, "traffic": traffic_of(args.workload, top),
+                     "traffic_source": "profiles/traffic.json (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)",
                      "peak_source": ("FP64 FMA micro-benchmark measured in this run (sph_measure_fp64_peak); nominal "
                                      "148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s") if roofline["bound"] == "alu"
                      else hbm_src})
@@ -524,7 +532,7 @@ def main():
                         "runs on every particle; value/ms_per_step above are the nominal t = 0 state of BASELINE.json",
                 "twin_stages_ms_per_eval": twin_stages,
                 "hbm_copy_gbs_this_run": round(r["copy_gbs"], 1),
-                "counters_last_eval": r["counters"]}),
+                "counters_per_eval": r["counters"]}),
             "clocks": r["clocks"],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(r["h2d"]),
                     "d2h_bytes_per_step": int(r["d2h"]), "ms_per_step": ms_e2e},
@@ -551,14 +559,17 @@ def main():
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures under profiles/ (filled in per round; None = not captured yet).
-TRAFFIC_NCU = {
-    # profiles/r2_c5.md: k_gravity<3,4,2,0,0> 0.318 GB read + 0.084 GB written per launch
-    ("C5", "gravity"): 402.6e6,
-    ("C5", "pairs"): 3152.5e6,          # profiles/r2_c5.md
-    ("C5", "neighbours"): 2755.4e6,
-}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of a stage's kernel: profiles/traffic.json, written from the
+# committed `ncu --set full` capture of the same kernels (the file names the capture); None = not captured.
+def traffic_of(workload, stage):
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)
+        e = t["kernels"].get(workload, {}).get(stage)
+        return None if e is None else float(e["dram_bytes_read"]) + float(e["dram_bytes_write"])
+    except (OSError, ValueError, KeyError):
+        return None
+
 
 if __name__ == "__main__":
     sys.exit(main())

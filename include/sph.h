@@ -229,10 +229,14 @@ int sph_download(sph_ctx *ctx, const sph_state_out *dst, int dst_is_device);
  * (every particle's density and smoothing length feed its partners' sums); the pair sums and the walk are still sharded.
  * sph_get_neighbours then returns the lists of the rank's own slice only; the work counters are per rank.  sph_step does
  * not capture CUDA graphs while a partition is set.
- * The device-side failure flags (list overflow, stack guards, largest partner count) are collective: every exchange carries
- * one more array of elem_bytes = 1 in which each rank's slot holds its flags, and after the all-gather every rank folds all
+ * The library packs the rank's slices of all exchanged arrays into one contiguous block first (one kernel), so the
+ * function is called with n_arrays = 1 -- ONE collective per evaluation, elem_bytes[0] = the bytes per particle of all
+ * arrays together (137 for a solid, damaged, self-gravitating run) -- and copies the other ranks' blocks back into the
+ * arrays afterwards (one kernel); a conforming function still handles any n_arrays.
+ * The device-side failure flags (list overflow, stack guards, largest partner count) are collective: the packed block also
+ * carries one byte per particle in which each rank's slot holds its flags, and after the all-gather every rank folds all
  * slots into its own, so that all ranks return the same error from the same call and sph_step_rk3 accepts or gives back a
- * step on all ranks alike.  The caller's exchange function needs no special case for it. */
+ * step on all ranks alike. */
 typedef int (*sph_exchange_fn)(void *user, void *cuda_stream, int n_arrays, void *const *arrays, const int32_t *elem_bytes,
                                int64_t slice_elems);
 int sph_partition(int64_t n, int world, int rank, int64_t *lo, int64_t *hi, int64_t *slice);

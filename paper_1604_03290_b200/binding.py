@@ -346,7 +346,8 @@ class Context:
     def set_partition(self, rank, world, group=None, exchange=None):
         """sph_set_partition.  Every rank must have uploaded the same full state.  The all-gather of the rate arrays
         at the end of an evaluation is `exchange(tensors, slice_bytes)` if given (tests emulate ranks with it), else
-        all_gather_slices over the torch.distributed group (NCCL: one in-place all-gather per array over NVLink)."""
+        all_gather_slices over the torch.distributed group.  The library packs the slices of all rate arrays into one
+        block before it calls back, so this is ONE in-place NCCL all-gather per evaluation over NVLink."""
         torch = self.torch
         if world <= 1:
             self._check(load_library().sph_set_partition(self.handle, 0, 1, EXCHANGE_FN(0), None))

@@ -45,6 +45,19 @@ bool cfg_ok(const sph_config *c) {
     return true;
 }
 
+// Bytes per particle of everything a sharded evaluation exchanges (the list of exchange_rates with which = 3): the
+// ranks' flag slots (1), drho du (16), dv (24), dS (48, solid), ddmg strain n_act_new (20, damage), dxs (24, XSPH),
+// grad v and C (144, exported), nb_cnt (4), ag (24, gravity).  Sizes the pack buffer Dev::xbuf.
+int exchange_bytes_per_particle(int flags) {
+    int b = 1 + 16 + 24 + 4;
+    if (flags & SPH_F_SOLID) b += 48;
+    if (flags & SPH_F_DAMAGE) b += 20;
+    if (flags & SPH_F_XSPH) b += 24;
+    if ((flags & SPH_F_SOLID) && (flags & SPH_F_EXPORT_GRADV)) b += 144;
+    if (flags & SPH_F_GRAVITY) b += 24;
+    return b;
+}
+
 // Fills d with pointers into base (or only measures when base == nullptr). Returns bytes used.
 size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     Bump b{base, 0};
@@ -113,6 +126,7 @@ size_t carve(const sph_config *c, char *base, Dev *d, Mats **mats_dev) {
     for (int a = 0; a < 3; ++a) z.dxs[a] = b.take<double>((c->flags & SPH_F_XSPH) ? np_ : 1);
     for (int k = 0; k < 9; ++k) { z.gradv[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); z.Cten[k] = b.take<double>((c->flags & SPH_F_EXPORT_GRADV) ? np_ : 1); }
     z.xstat = b.take<unsigned char>(np_);
+    z.xbuf = b.take<unsigned char>(np_ * (size_t)exchange_bytes_per_particle(c->flags));
     Mats *md = b.take<Mats>(1);
     if (mats_dev) *mats_dev = md;
     if (d) *d = z;
@@ -705,17 +719,41 @@ __global__ void k_status_merge(Dev d, const unsigned char *xstat, i64 slice, int
     d.status->err_nb_overflow = ov; d.status->err_stack = stk; d.status->nb_max = mx;
 }
 
+// ONE all-gather per exchange: the rank's slices of all arrays are packed into one contiguous block of Dev::xbuf
+// (rank-major: block r = [array 0 slice | array 1 slice | ...] of rank r), the caller's function gathers that one array,
+// and the other ranks' blocks are copied back into the arrays.  A slice of `slice` elements of 1, 4 or 8 bytes is a whole
+// number of 32-byte pieces (slice is a multiple of 32) and every array starts on a 256-byte boundary, so both kernels
+// move 16-byte words.
+#define XJ_MAX 64
+struct XJobs {
+    unsigned char *arr[XJ_MAX];     // the array (element 0)
+    unsigned off[XJ_MAX];           // bytes per particle of the arrays before it
+    unsigned eb[XJ_MAX];            // its element size
+};
+// grid (pieces, arrays, ranks): unpack = 1 copies block q of xbuf into the arrays for every q but `rank`;
+// unpack = 0 copies the arrays' slices of `rank` into its block (gridDim.z = 1).
+__global__ void k_xcopy(XJobs jobs, unsigned char *xbuf, i64 slice, int sum_eb, int rank, int unpack) {
+    const int k = blockIdx.y;
+    const int q = unpack ? (int)blockIdx.z : rank;
+    if (unpack && q == rank) return;
+    const i64 words = slice * (i64)jobs.eb[k] / 16;
+    const i64 j = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= words) return;
+    uint4 *a = reinterpret_cast<uint4 *>(jobs.arr[k] + (size_t)q * (size_t)slice * jobs.eb[k]) + j;
+    uint4 *x = reinterpret_cast<uint4 *>(xbuf + (size_t)q * (size_t)slice * (size_t)sum_eb + (size_t)jobs.off[k] * (size_t)slice) + j;
+    if (unpack) *a = *x; else *x = *a;
+}
+
 // which: 1 = the arrays sph_rhs fills, 2 = the gravitational acceleration, 3 = both
 static int exchange_rates(sph_ctx *ctx, int which) {
     if (ctx->world <= 1 || !ctx->xfn) return SPH_OK;
     Dev &d = ctx->d;
-    void *arr[64];
-    int32_t eb[64];
+    XJobs jobs;
     int na = 0;
-    auto add = [&](void *p, int bytes) { arr[na] = p; eb[na] = bytes; ++na; };
+    unsigned sum_eb = 0;
+    auto add = [&](void *p, int bytes) { jobs.arr[na] = (unsigned char *)p; jobs.eb[na] = (unsigned)bytes; jobs.off[na] = sum_eb; sum_eb += bytes; ++na; };
     // slice is a multiple of 32, so a slot of `slice` BYTES holds the three words and keeps them 4-byte aligned
     k_status_pack<<<1, 1, 0, ctx->stream>>>(d, reinterpret_cast<int *>(d.xstat + (size_t)ctx->rank * (size_t)ctx->slice));
-    ctx->launches += 1;
     add(d.xstat, 1);
     if (which & 1) {
         add(d.drho, 8); add(d.du, 8);
@@ -728,10 +766,15 @@ static int exchange_rates(sph_ctx *ctx, int which) {
         add(d.nb_cnt, 4);
     }
     if ((which & 2) && (d.flags & SPH_F_GRAVITY)) for (int a = 0; a < 3; ++a) add(d.ag[a], 8);
-    if (ctx->xfn(ctx->xuser, (void *)ctx->stream, na, arr, eb, (int64_t)ctx->slice) != 0)
+    const int pieces = sph_ceil_div(ctx->slice * 8 / 16, 256);         // of the widest element; narrower arrays exit early
+    k_xcopy<<<dim3(pieces, na, 1), 256, 0, ctx->stream>>>(jobs, d.xbuf, ctx->slice, (int)sum_eb, ctx->rank, 0);
+    void *arr[1] = {d.xbuf};
+    int32_t eb[1] = {(int32_t)sum_eb};
+    if (ctx->xfn(ctx->xuser, (void *)ctx->stream, 1, arr, eb, (int64_t)ctx->slice) != 0)
         return fail(ctx, SPH_ERR_CUDA, "the caller's exchange function (all-gather of the rates) failed");
+    k_xcopy<<<dim3(pieces, na, ctx->world), 256, 0, ctx->stream>>>(jobs, d.xbuf, ctx->slice, (int)sum_eb, ctx->rank, 1);
     k_status_merge<<<1, 1, 0, ctx->stream>>>(d, d.xstat, ctx->slice, ctx->world);
-    ctx->launches += 1;
+    ctx->launches += 4;
     return SPH_OK;
 }
 

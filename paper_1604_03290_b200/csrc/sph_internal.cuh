@@ -138,6 +138,7 @@ struct Dev {
     int *n_act_new;
     // ---- sharding: the ranks' failure flags travel with the rates (api.cu exchange_rates) ----
     unsigned char *xstat;       // world * slice bytes; rank r's slot = 3 ints at byte r * slice
+    unsigned char *xbuf;        // pack buffer of the ONE all-gather per exchange: world blocks of slice * (bytes per particle)
 };
 
 struct SphTiming;   // api.cu: CUDA-event pairs around the stages (sph_timing_*)

@@ -720,6 +720,7 @@ class VirtualRanks:
         self.slots = [None] * world
         self.errors = []
         self.ctx = []
+        self.calls = [[] for _ in range(world)]                  # per rank: number of arrays of every exchange call
         for r in range(world):
             cfg, mats = P.config_of(w, **kw)
             c = P.sph_create(cfg, mats, stream=torch.cuda.Stream())
@@ -731,6 +732,7 @@ class VirtualRanks:
         torch = self.torch
 
         def ex(tensors, slice_bytes):
+            self.calls[r].append(len(tensors))
             torch.cuda.current_stream().synchronize()            # my slices are complete
             self.slots[r] = tensors
             self.bar.wait()
@@ -792,6 +794,8 @@ def test_sharded_evaluation_and_step_equal_single_gpu_bit_for_bit(P, name, world
         return a, ctx.download(), nb
 
     res = vr.run(job)
+    # ONE collective per evaluation (the slices of all arrays travel as one packed block): 1 + 2 x 2 evaluations
+    assert vr.calls == [[1] * 5] * world, vr.calls
     off_all, idx_all = [], []
     for r, (a, b, (off, idx)) in enumerate(res):
         for k in want_eval:                                       # every rank ends with the complete arrays
