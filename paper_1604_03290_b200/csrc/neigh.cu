@@ -36,9 +36,7 @@
 #define NB_WARPS 2
 #define NB_STACK 384            // ranges of child items per warp
 #define NB_RESERVE 168          // a depth-first descent keeps <= 8 pending siblings per tree level (21 levels)
-#ifndef NB_RANGES
 #define NB_RANGES 4             // ranges (cells) whose child items one round tests
-#endif
 
 // ------------------------------------------------------------------------------------------
 // search tree

@@ -10,9 +10,7 @@
 #include "sph_internal.cuh"
 
 #define SORT_THREADS 256
-#ifndef SORT_ITEMS
 #define SORT_ITEMS 8                    // measured on C5: 16 -> 0.556 ms, 12 -> 0.520, 8 -> 0.517 (shorter ranking chains, 6 blocks per SM)
-#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_WARPS (SORT_THREADS / 32)
 

@@ -197,12 +197,8 @@ __device__ __forceinline__ double max_eig_sym(double a00, double a01, double a02
     }
 }
 
-#ifndef PR_WARPS
 #define PR_WARPS 1
-#endif
-#ifndef PR_MINBLOCKS
 #define PR_MINBLOCKS 1            // resident blocks per SM the register allocation must allow (1 = no cap)
-#endif
 #define PR_STRIDE 18            // doubles between staged records (144 B): 16-byte reads by lane are conflict-free
 
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src) {

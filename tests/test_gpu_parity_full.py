@@ -16,7 +16,8 @@ import pytest
 
 import sph_inputs
 from oracle import oracle as orc
-from test_gpu_parity import P, assert_close, canonical, check_rates, make_ctx  # noqa: F401
+from test_gpu_parity import (P, VirtualRanks, assert_close, canonical, check_neighbours, check_rates,  # noqa: F401
+                             make_ctx, n_act_tie_zone)
 
 pytestmark = pytest.mark.gpu
 
@@ -131,4 +132,133 @@ def test_c1_full_size(P):
     assert np.array_equal(off, o["nb_off"]) and np.array_equal(idx, o["nb_idx"])
     check_rates(w, ctx.download(), o)
     assert np.bincount(np.diff(off)).argmax() == 20
+    ctx.close()
+
+
+def test_c1x_full_size(P):
+    """The paper's own ring test (artificial stress + XSPH) at its full 4 416 particles, brute force."""
+    w = sph_inputs.make("C1x", twin=True)
+    ctx = make_ctx(P, w, h_iters=0)
+    ctx.evaluate()
+    o = orc.evaluate(w, mode="brute", h_iters=0)
+    off, idx = ctx.get_neighbours()
+    assert np.array_equal(off, o["nb_off"]) and np.array_equal(idx, o["nb_idx"])
+    check_rates(w, ctx.download(), o)
+    ctx.close()
+
+
+@pytest.mark.parametrize("unconverge", [False, True])
+def test_c2_full_size_timed_configuration(P, unconverge):
+    """C2 as bench.py times it: h_iters = 1, i.e. eq. 73 on and three tree walks per evaluation
+    (count by own h, the symmetric search, the walk for self-gravity), for all 65 536 particles.  The workload's h is a
+    fixed point of eq. 73 (every particle has n_des partners inside its own h), so the timed configuration leaves h
+    unchanged; the second case scatters h by -15 .. +20 % first so that the update moves every particle.  The new h
+    agrees up to the ulp of cbrt (reading U5): CUDA's and glibc's cbrt are each within 1 ulp of the exact root, so they
+    differ by at most 2 ulp(c) <= 4.4e-16; h_new = (h/2)(1 + c) with 1 + c in [1.5, 3) then carries that as <= 3e-16
+    relative plus one rounding of the sum and one of the product on either side (4 x 1.1e-16): 8e-16 relative is the
+    bound, 4.2e-16 the largest seen over the 65 536 particles (the 2 500-particle case stays inside 4e-16).  Where h
+    differs the partner sets are checked against the oracle's search run on the GPU's h, as in
+    test_variable_h_update_eq73."""
+    w = sph_inputs.make("C2", twin=True)
+    assert w.h_iters == 1
+    if unconverge:
+        w.h = w.h * np.random.default_rng(2).uniform(0.85, 1.2, w.n)
+    ctx = make_ctx(P, w)                                     # the workload's own h_iters, as bench.py's config_of(w)
+    ctx.evaluate()
+    g = ctx.download()
+    o = orc.evaluate(w, mode="tree")
+    assert_close("h", g["h"], o["h"], rel=8e-16)
+    assert np.array_equal(o["h"], w.h) != unconverge         # fixed point / every h moved
+    if np.array_equal(g["h"], o["h"]):
+        check_neighbours(ctx, o["nb_off"], o["nb_idx"])
+    else:
+        w2 = w.copy(); w2.h = g["h"]
+        off, idx = orc.neighbours(w2, mode="tree")
+        check_neighbours(ctx, off, idx)
+    check_rates(w, g, o)
+    c = ctx.get_counters()
+    assert (c["n_inter"], c["n_visit"], c["n_open"]) == (o["n_inter"].sum(), o["n_test"].sum(), o["n_open"].sum())
+    ctx.close()
+
+
+_BIG = {}
+
+
+def _big_c5():
+    """C5 at scale 0.2 (800 014 particles): a slice of 2 or 3 ranks stays above the 200 000 particles from which the walk
+    takes 16 particles per warp (gravity.cu GR_PPW_FROM), the sort has hundreds of tiles."""
+    if "w" not in _BIG:
+        _BIG["w"] = sph_inputs.make("C5", scale=0.2, twin=True)
+    return _BIG["w"]
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_slices_above_the_wide_walk_threshold(P, world):
+    """Morton-range sharding where a slice boundary meets the 16-particles-per-warp walk and a multi-tile sort: every rank
+    ends an evaluation and a step with the single-GPU arrays, bit for bit."""
+    w = _big_c5()
+    lo, hi, _ = P.sph_partition(w.n, world, world - 1)
+    assert hi - lo >= 200_000
+    if "want" not in _BIG:
+        single = make_ctx(P, w, h_iters=0)
+        single.evaluate()
+        a = single.download()
+        single.step(w.dt)
+        _BIG["want"] = (a, single.download())
+        single.close()
+    want_eval, want_step = _BIG["want"]
+    vr = VirtualRanks(P, w, world, h_iters=0)
+
+    def job(ctx):
+        ctx.evaluate()
+        a = ctx.download()
+        ctx.step(w.dt)
+        return a, ctx.download()
+
+    for r, (a, b) in enumerate(vr.run(job)):
+        for k in want_eval:
+            assert np.array_equal(a[k], want_eval[k]), (r, "evaluate", k)
+        for k in want_step:
+            assert np.array_equal(b[k], want_step[k]), (r, "step", k)
+    assert vr.calls == [[1] * 3] * world
+    vr.close()
+
+
+def test_rk3_and_decoupled_gravity_at_full_size_c6(P):
+    """sph_step_rk3 (eqs. 58-65) and gravity_every = 2 (reading U31) on all 400 116 particles of C6, the
+    oracle's tree mode as the checker: the kernels run in the configuration of the large workloads (wide walk, many sort
+    tiles), which the 3 000-particle cases of test_gpu_parity.py do not reach."""
+    w = sph_inputs.make("C6", twin=True)
+    w.flags |= P.SPH_F_RK3
+    w0 = w.copy(); w0.h_iters = 0
+    qn, err_o, dt_o, ok_o, fs = orc.step_rk3(w0, w.dt, 1e30, mode="tree")
+    assert ok_o
+    ctx = make_ctx(P, w, h_iters=0)
+    err, dt_new, ok = ctx.step_rk3(w.dt, 1e30)
+    assert ok
+    assert err == pytest.approx(err_o, rel=1e-6) and dt_new == pytest.approx(dt_o, rel=1e-6)
+    g = ctx.download(P.STATE_FIELDS)
+    for k in ("x", "v", "rho", "u", "S", "dmg"):
+        go, oo = g[k], getattr(qn, k)
+        scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
+        assert np.all(np.abs(go - oo) <= 1e-9 * np.abs(oo) + 1e-12 * scale), k
+    n_act_tie_zone(w, g["n_act"], qn.n_act, np.maximum(np.maximum(fs[0]["strain"], fs[1]["strain"]), fs[2]["strain"]), rel=1e-8)
+    ctx.close()
+    # decoupled gravity: step 0 walks, step 1 takes the stored field of step 0's second evaluation
+    cfg, mats = P.config_of(w, h_iters=0, gravity_every=2)
+    ctx = P.sph_create(cfg, mats)
+    ctx.upload_workload(w)
+    q = w.copy(); q.h_iters = 0
+    keep = None
+    for s in range(2):
+        ctx.step(w.dt)
+        q, f1, f2 = orc.step(q, w.dt, mode="tree", ag_reuse=None if s == 0 else keep)
+        keep = f2["ag"].copy()
+        q.h_iters = 0
+        g = ctx.download()
+        for k in ("x", "v", "rho", "u", "S", "dmg"):
+            go, oo = g[k], getattr(q, k)
+            scale = np.abs(oo).max() if np.abs(oo).max() > 0 else 1.0
+            assert np.all(np.abs(go - oo) <= 1e-8 * np.abs(oo) + 1e-11 * scale), (s, k)
+        assert_close(f"ag(step {s})", g["ag"], f2["ag"], rel=1e-8, floor=1e-11 * np.abs(f2["ag"]).max())
     ctx.close()
